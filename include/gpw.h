@@ -1,0 +1,165 @@
+/*
+ * gpw.h -- C ABI of the B200-native multigrid Gaussian-Plane-Wave hot path.
+ *
+ * Operations (citations are lines of the paper's text, /root/reference/PAPER.md,
+ * with the equation / algorithm they fall in; "DESIGN.md Tn / An" are the
+ * readings of the paper listed in DESIGN.md):
+ *
+ *   gpw_build_pairs   shell cutoff radii (Eq. 20), pair screening
+ *                     and lattice-image lists (Eq. 18-19; Alg. 4,
+ *                     PAPER.md:435-479), level assignment by pair exponent
+ *                     (PAPER.md:59), pair -> 4x4x4 grid-block lists (Alg. 5,
+ *                     PAPER.md:485-561).
+ *   gpw_eval_rho      density collocation, Eq. (3) PAPER.md:41 / Alg. 1
+ *                     PAPER.md:204-234, on every level's grid; deriv=1 adds the
+ *                     exact real-space gradient (Eq. 10 is its G-space form,
+ *                     PAPER.md:76-82).
+ *   gpw_eval_mat      potential integration, Eq. (4) PAPER.md:45 with the quadrature
+ *                     weight of Eq. (29) PAPER.md:185 / Alg. 2 PAPER.md:240-263;
+ *                     deriv=1 adds the Eq. (11) term sum_r w(r) . grad(phi_mu phi_nu)
+ *                     (before the integration by parts of Eq. 13).
+ *   gpw_interp_up / gpw_restrict_down
+ *                     inter-level Fourier combination, Eq. (7)-(8) PAPER.md:61-68
+ *                     (cuFFT, off the optimisation target).
+ *
+ * Conventions
+ *   - All functions return GPW_OK (0) or a negative gpw_status; they never throw,
+ *     exit or print.  gpw_last_error() gives a thread-local message.
+ *   - "host" / "device" on every pointer says where the memory lives.  The caller
+ *     owns every buffer it passes; the library copies what it needs into the plan
+ *     and keeps no caller pointer after a call returns.
+ *   - Basis (Eq. 21-22): primitive k of a shell of angular
+ *     momentum l centred at A is coef_k x^lx y^ly z^lz exp(-a_k |r-A|^2),
+ *     lx+ly+lz = l; coef multiplies the bare primitive as is (normalisation is the
+ *     caller's business, A1).  AO order: shells in input order, within a
+ *     shell the Cartesian components with decreasing lx, then decreasing ly
+ *     (s; x y z; xx xy xz yy yz zz; xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz; A2).
+ *   - Grids (PAPER.md:483 with u0 = 0): level alpha has mesh (N1,N2,N3), points
+ *     r_n = (n1/N1) a1 + (n2/N2) a2 + (n3/N3) a3; arrays are [ncomp][N1][N2][N3]
+ *     doubles, C order (n3 fastest), ncomp = 1 (deriv=0) or 4 (deriv=1: value,
+ *     d/dx, d/dy, d/dz; component-major).
+ *   - Truncation (T1-T7): a primitive pair is evaluated on all 64 points
+ *     of every aligned 4x4x4 grid block that has at least one point within the pair
+ *     radius R_t of the Gaussian-product centre; out-of-cell blocks are folded back
+ *     (Eq. 18-19).
+ *   - eval calls are asynchronous on the given CUDA stream, allocate nothing
+ *     visible to the caller and do not synchronise.  Results may differ from run to
+ *     run at the 1e-15 level (floating-point atomics).
+ */
+#ifndef GPW_H
+#define GPW_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GPW_MAX_LEVEL 8
+#define GPW_MAX_L 3
+
+typedef struct gpw_plan gpw_plan; /* opaque; owned by the library; freed by gpw_free_plan */
+
+typedef enum {
+    GPW_OK = 0,
+    GPW_EINVAL = -1,       /* null pointer, l > 3, exponent/tau <= 0, singular cell (|det| < 1e-12),
+                              mesh entry not a positive multiple of 4, deriv not in {0,1}, nlevel > 8 */
+    GPW_ENOMEM = -2,
+    GPW_ECUDA = -3,        /* a CUDA / cuFFT call failed, or the plan has no device copy */
+    GPW_EUNSUPPORTED = -4  /* l >= 4, more lattice wraps than the visit encoding holds */
+} gpw_status;
+
+/* Plan summary (host struct filled by gpw_plan_info). */
+typedef struct {
+    int nao, nshl, nlevel, hermi, on_device;
+    long ntask;                               /* primitive pairs (a, b, T) kept (unordered if hermi) */
+    long ntask_level[GPW_MAX_LEVEL];
+    long nvisit_level[GPW_MAX_LEVEL];         /* (pair, 4x4x4 block) visits */
+    long nvisit_class[GPW_MAX_LEVEL][GPW_MAX_L + 1][GPW_MAX_L + 1]; /* per (la, lb); points = 64 * visits */
+    long nitem;                               /* work items (block, visit range) of the kernels */
+    long ncoef_total;                         /* doubles in the per-pair polynomial workspace */
+    double build_seconds;                     /* host time spent in gpw_build_pairs */
+    long device_bytes;                        /* device memory held by the plan */
+} gpw_info;
+
+/* One kept primitive pair (host struct filled by gpw_plan_export_tasks). */
+typedef struct {
+    int shl_a, prim_a, shl_b, prim_b;  /* shell index, global primitive index */
+    int T[3];                          /* lattice translation applied to b */
+    int level;
+    double R;                          /* pair radius R_t (T4) */
+} gpw_task;
+
+/*
+ * Screening, radii, level assignment, lattice images and block lists.
+ * All pointer arguments are HOST memory.
+ *   cell        [9]  row-major, rows = lattice vectors a1, a2, a3 (Bohr)
+ *   xyz         [natm][3] Bohr, used as given (need not lie inside the cell)
+ *   shl_atom    [nshl] centre index;  shl_l [nshl] 0..3;  shl_nprim [nshl] >= 1;
+ *   shl_prim_off[nshl] offset of the shell's first primitive in prim_exp / prim_coef
+ *   prim_exp    [nprim] Bohr^-2, > 0;  prim_coef [nprim]
+ *   mesh        [nlevel][3], finest level first, every entry a positive multiple of 4
+ *   tau         threshold of Eq. (20);  rel_cutoff  level-assignment constant (T5):
+ *               a pair goes to the coarsest level with E_alpha >= rel_cutoff * a_p
+ *   hermi       1: D and F symmetric, unordered pairs processed once;  0: ordered pairs
+ * On success *plan_out holds a plan with a device copy on the current CUDA device.
+ * If no CUDA device is usable the plan is host-only (info.on_device = 0): it serves
+ * gpw_plan_info / gpw_plan_export_tasks, and every eval call on it fails with
+ * GPW_ECUDA (there is no CPU fallback).  May synchronise the device.
+ */
+int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
+                    const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
+                    const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
+                    double tau, double rel_cutoff, int hermi, gpw_plan **plan_out);
+
+/*
+ * Collocation.  D_dev: DEVICE [nao][nao] row-major (read only).  deriv: 0 or 1.
+ * rho_dev: HOST array of nlevel DEVICE pointers, each [ncomp][N1][N2][N3]; every level
+ * is OVERWRITTEN (levels without pairs are zero-filled).  cuda_stream: a cudaStream_t
+ * (NULL = default stream).  With hermi = 1 the pair (a,b) uses D_ab + D_ba, so the
+ * result equals the ordered double sum of Eq. (3) for any D.
+ */
+int gpw_eval_rho(const gpw_plan *plan, const double *D_dev, int deriv, double *const *rho_dev,
+                 void *cuda_stream);
+
+/*
+ * Integration.  v_dev: HOST array of nlevel DEVICE pointers, each [ncomp][N1][N2][N3]
+ * (component 0 = v, components 1..3 = the vector field w contracted with
+ * grad(phi_mu phi_nu)).  F_dev: DEVICE [nao][nao] row-major, OVERWRITTEN, includes
+ * dV = Omega / (N1 N2 N3) of each level and the sum over levels.  With hermi = 1 both
+ * triangles are written.
+ */
+int gpw_eval_mat(const gpw_plan *plan, const double *const *v_dev, int deriv, double *F_dev,
+                 void *cuda_stream);
+
+/*
+ * Off-target helpers (cuFFT), Eq. (7)-(8):
+ *   up:   rho_fine = IFFT( sum_alpha [FFT(rho_alpha)]_{|G| < G_alpha} ) on the finest mesh
+ *   down: v_alpha  = IFFT( [FFT(v_fine)]_{|G| < G_alpha} )   (the exact adjoint of up)
+ * G_alpha = min_i pi N_alpha,i |b_i| (inscribed sphere; excludes Nyquist planes; A17).
+ * rho_dev / v_dev: HOST arrays of nlevel DEVICE pointers [ncomp][N1][N2][N3];
+ * rho_fine_dev / v_fine_dev: DEVICE [ncomp] arrays on the finest (level 0) mesh.
+ * These allocate cuFFT plans and scratch inside the plan on first use.
+ */
+int gpw_interp_up(gpw_plan *plan, const double *const *rho_dev, int ncomp, double *rho_fine_dev,
+                  void *cuda_stream);
+int gpw_restrict_down(gpw_plan *plan, const double *v_fine_dev, int ncomp, double *const *v_dev,
+                      void *cuda_stream);
+
+/* Introspection (host). */
+int gpw_plan_info(const gpw_plan *plan, gpw_info *out);
+/* Copies up to cap tasks into host_buf (may be NULL with cap = 0); *ntask = total. */
+int gpw_plan_export_tasks(const gpw_plan *plan, gpw_task *host_buf, long cap, long *ntask);
+
+/*
+ * Measurement aid: FP64 FMA throughput of the current device (register-only DFMA loop on every SM, 8
+ * independent chains per thread, best launch over at least min_seconds), in TFLOP/s.  The denominator
+ * of the "alu" roofline that bench.py reports.  Host pointers; synchronises the device.
+ */
+int gpw_dfma_peak(double min_seconds, double *tflops_out, int *sm_count_out);
+
+void gpw_free_plan(gpw_plan *plan);
+const char *gpw_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPW_H */

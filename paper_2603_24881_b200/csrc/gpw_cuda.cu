@@ -1,0 +1,554 @@
+// CUDA kernels (sm_100a) and the C ABI of include/gpw.h.
+//
+// Kernels:
+//   k_poly_from_D       pre-pass: one thread per pair, D block -> polynomial about P in grid-index coordinates
+//   k_collocate<DERIV>  Eq. (3): one warp per work item (a 4x4x4 block and a range of its visit list);
+//                       a half-warp evaluates one (pair, block) visit, a lane owns a column of 4 points
+//                       and keeps its rho values in registers; one store (or atomic add) per point at the end
+//   k_integrate<DERIV>  Eq. (4): same decomposition; the block of v lives in registers, each visit's
+//                       moment vector is reduced over the half-warp by a shuffle reduce-scatter and added
+//                       to the pair's moment vector
+//   k_F_from_moments    post-pass: one thread per pair, moments -> F block (x dV), atomics into F
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gpw_math.cuh"
+
+namespace gpw {
+const char *last_error_cstr();
+
+struct GridParams {
+    LevelGeom lev[GPW_MAX_LEVEL];
+    const long long *tile_base[GPW_MAX_LEVEL];
+    const unsigned *seg[GPW_MAX_LEVEL];
+    double *grid[GPW_MAX_LEVEL];   // rho (written) or v (read)
+};
+
+// ------------------------------------------------------------------------------------------ pre/post pass
+__global__ void __launch_bounds__(128) k_poly_from_D(const TaskP *__restrict__ tp, int ntask,
+                                                      const double *__restrict__ D, int nao,
+                                                      const double *__restrict__ S_all, double *__restrict__ coef) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntask) return;
+    const TaskP p = tp[t];
+    pair_poly_from_D(p, D, nao, S_all + (size_t)p.level * S_TOTAL, coef + p.coef_off);
+}
+
+struct DVs { double v[GPW_MAX_LEVEL]; };
+
+__global__ void __launch_bounds__(128) k_F_from_moments(const TaskP *__restrict__ tp, int ntask,
+                                                         const double *__restrict__ mom,
+                                                         const double *__restrict__ S_all, DVs dV,
+                                                         double *__restrict__ F, int nao) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntask) return;
+    const TaskP p = tp[t];
+    double blk[ncart(MAXL) * ncart(MAXL)];
+    pair_block_from_moments(p, mom + p.coef_off, S_all + (size_t)p.level * S_TOTAL, dV.v[p.level], blk);
+    const int nca = ncart(p.la), ncb = ncart(p.lb);
+    for (int i = 0; i < nca; i++)
+        for (int j = 0; j < ncb; j++) {
+            const double x = blk[i * ncb + j];
+            atomicAdd(F + (size_t)(p.ao_a + i) * nao + p.ao_b + j, x);
+            if (p.sym) atomicAdd(F + (size_t)(p.ao_b + j) * nao + p.ao_a + i, x);
+        }
+}
+
+// ------------------------------------------------------------------------------------------ collocation
+struct VisitCtx {
+    const TaskK *tasks;
+    const Visit *visits;   // already offset to the block's list
+    const double *work;    // polynomial workspace
+    double gm[6];
+    int n1, n2, n3;        // stored index of the lane's column start
+    int N0, N1, N2;
+};
+
+struct LoadedVisit {
+    double u1, u2, u30, ap, cc;
+    long long coef_off;
+};
+
+__device__ __forceinline__ LoadedVisit load_visit(const VisitCtx &c, unsigned v) {
+    const Visit vi = c.visits[v];
+    const double2 *tk = reinterpret_cast<const double2 *>(c.tasks + vi.task);
+    const double2 a = __ldg(tk), b = __ldg(tk + 1), d = __ldg(tk + 2);
+    LoadedVisit r;
+    r.u1 = (double)(c.n1 + vi.s[0] * c.N0) - a.x;
+    r.u2 = (double)(c.n2 + vi.s[1] * c.N1) - a.y;
+    r.u30 = (double)(c.n3 + vi.s[2] * c.N2) - b.x;
+    r.ap = b.y;
+    r.cc = d.x;
+    r.coef_off = __double_as_longlong(d.y);
+    return r;
+}
+
+template <int L, int DERIV>
+__device__ __forceinline__ void colloc_segment(const VisitCtx &c, unsigned lo, unsigned hi, int half,
+                                               double (*acc)[4]) {
+    for (unsigned v = lo + half; v < hi; v += 2) {
+        const LoadedVisit lv = load_visit(c, v);
+        double q[6];
+#pragma unroll
+        for (int x = 0; x < 6; x++) q[x] = lv.ap * c.gm[x];
+        colloc_column<L, DERIV>(c.work + lv.coef_off, q, lv.cc, lv.u1, lv.u2, lv.u30, acc);
+    }
+}
+
+template <int DERIV>
+__global__ void __launch_bounds__(128) k_collocate(const __grid_constant__ GridParams P,
+                                                    const TaskK *__restrict__ tasks,
+                                                    const Visit *__restrict__ visits,
+                                                    const Item *__restrict__ items, int nitem,
+                                                    const double *__restrict__ coef) {
+    constexpr int NCOMP = DERIV ? 4 : 1;
+    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (w >= nitem) return;
+    const Item it = items[w];
+    const LevelGeom &g = P.lev[it.level];
+    const int lane = threadIdx.x & 31, half = lane >> 4, col = lane & 15;
+    const int T2 = g.T[2], T1 = g.T[1];
+    const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
+    VisitCtx c;
+    c.tasks = tasks;
+    c.visits = visits + P.tile_base[it.level][it.tile];
+    c.work = coef;
+#pragma unroll
+    for (int x = 0; x < 6; x++) c.gm[x] = g.Gm[x];
+    c.n1 = 4 * b1 + (col >> 2); c.n2 = 4 * b2 + (col & 3); c.n3 = 4 * b3;
+    c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
+    const unsigned *seg = P.seg[it.level] + (size_t)it.tile * 8;
+
+    double acc[NCOMP][4];
+#pragma unroll
+    for (int k = 0; k < NCOMP; k++)
+#pragma unroll
+        for (int t = 0; t < 4; t++) acc[k][t] = 0.0;
+
+#pragma unroll 1
+    for (int L = 0; L <= MAXLP; L++) {
+        const unsigned lo = max(it.lo, seg[L]), hi = min(it.hi, seg[L + 1]);
+        if (lo >= hi) continue;
+        switch (L) {
+            case 0: colloc_segment<0, DERIV>(c, lo, hi, half, acc); break;
+            case 1: colloc_segment<1, DERIV>(c, lo, hi, half, acc); break;
+            case 2: colloc_segment<2, DERIV>(c, lo, hi, half, acc); break;
+            case 3: colloc_segment<3, DERIV>(c, lo, hi, half, acc); break;
+            case 4: colloc_segment<4, DERIV>(c, lo, hi, half, acc); break;
+            case 5: colloc_segment<5, DERIV>(c, lo, hi, half, acc); break;
+            default: colloc_segment<6, DERIV>(c, lo, hi, half, acc); break;
+        }
+    }
+    // the two half-warps worked on alternate visits of the same block
+#pragma unroll
+    for (int k = 0; k < NCOMP; k++)
+#pragma unroll
+        for (int t = 0; t < 4; t++) acc[k][t] += __shfl_xor_sync(0xffffffffu, acc[k][t], 16);
+    if (half) return;
+    const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
+    double *out = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2) * g.N[2] + c.n3;
+    double res[NCOMP][4];
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+        res[0][t] = acc[0][t];
+        if constexpr (DERIV) {
+            // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i
+#pragma unroll
+            for (int x = 0; x < 3; x++)
+                res[1 + x][t] = g.Hinv[0 * 3 + x] * acc[1][t] + g.Hinv[1 * 3 + x] * acc[2][t] +
+                                g.Hinv[2 * 3 + x] * acc[3][t];
+        }
+    }
+    if (it.single) {
+#pragma unroll
+        for (int k = 0; k < NCOMP; k++) {
+            double2 *o = reinterpret_cast<double2 *>(out + k * ng);
+            o[0] = make_double2(res[k][0], res[k][1]);
+            o[1] = make_double2(res[k][2], res[k][3]);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < NCOMP; k++)
+#pragma unroll
+            for (int t = 0; t < 4; t++) atomicAdd(out + k * ng + t, res[k][t]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ integration
+// Sum an N-vector held by each of the 16 lanes of a half-warp; afterwards lane j holds elements
+// [j*N/16, (j+1)*N/16) of the total in m[0 .. N/16).  N is a multiple of 16.
+template <int N>
+__device__ __forceinline__ void halfwarp_reduce_scatter(double *m, int lane) {
+    static_assert(N % 16 == 0, "pad to a multiple of 16");
+#pragma unroll
+    for (int step = 0; step < 4; step++) {
+        const int bit = 8 >> step;
+        const int len = N >> (step + 1);
+        const bool up = lane & bit;
+#pragma unroll
+        for (int i = 0; i < len; i++) {
+            const double send = up ? m[i] : m[i + len];
+            const double keep = up ? m[i + len] : m[i];
+            m[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
+        }
+    }
+}
+
+template <int L, int DERIV>
+__device__ __forceinline__ void integ_segment(const VisitCtx &c, unsigned lo, unsigned hi, int lane,
+                                              const double (*vv)[4], double *__restrict__ mom) {
+    constexpr int NC = ncoef(L);
+    constexpr int NPAD = (NC + 15) / 16 * 16;
+    constexpr int PER = NPAD / 16;
+    const int half = lane >> 4;
+    for (unsigned v0 = lo; v0 < hi; v0 += 2) {   // warp-uniform trip count: the shuffles need every lane
+        const unsigned v = v0 + half;
+        const bool active = v < hi;
+        const LoadedVisit lv = load_visit(c, active ? v : lo);
+        double q[6];
+#pragma unroll
+        for (int x = 0; x < 6; x++) q[x] = lv.ap * c.gm[x];
+        double m[NPAD];
+#pragma unroll
+        for (int i = 0; i < NPAD; i++) m[i] = 0.0;
+        integ_column<L, DERIV>(vv, q, lv.cc, lv.u1, lv.u2, lv.u30, m);
+        halfwarp_reduce_scatter<NPAD>(m, lane);
+        if (active) {
+            double *dst = mom + lv.coef_off + (lane & 15) * PER;
+#pragma unroll
+            for (int i = 0; i < PER; i++)
+                if ((lane & 15) * PER + i < NC) atomicAdd(dst + i, m[i]);
+        }
+    }
+}
+
+template <int DERIV>
+__global__ void __launch_bounds__(128) k_integrate(const __grid_constant__ GridParams P,
+                                                    const TaskK *__restrict__ tasks,
+                                                    const Visit *__restrict__ visits,
+                                                    const Item *__restrict__ items, int nitem,
+                                                    double *__restrict__ mom) {
+    constexpr int NCOMP = DERIV ? 4 : 1;
+    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (w >= nitem) return;
+    const Item it = items[w];
+    const LevelGeom &g = P.lev[it.level];
+    const int lane = threadIdx.x & 31, col = lane & 15;
+    const int T2 = g.T[2], T1 = g.T[1];
+    const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
+    VisitCtx c;
+    c.tasks = tasks;
+    c.visits = visits + P.tile_base[it.level][it.tile];
+    c.work = nullptr;
+#pragma unroll
+    for (int x = 0; x < 6; x++) c.gm[x] = g.Gm[x];
+    c.n1 = 4 * b1 + (col >> 2); c.n2 = 4 * b2 + (col & 3); c.n3 = 4 * b3;
+    c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
+    const unsigned *seg = P.seg[it.level] + (size_t)it.tile * 8;
+
+    // the lane's column of v; for DERIV the vector field is mapped to grid-index components,
+    // w'_i = sum_c Hinv[i][c] w_c, so that w . grad_r f = w' . grad_u f
+    const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
+    const double *in = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2) * g.N[2] + c.n3;
+    double raw[NCOMP][4], vv[NCOMP][4];
+#pragma unroll
+    for (int k = 0; k < NCOMP; k++) {
+        const double2 *p2 = reinterpret_cast<const double2 *>(in + k * ng);
+        const double2 x0 = __ldg(p2), x1 = __ldg(p2 + 1);
+        raw[k][0] = x0.x; raw[k][1] = x0.y; raw[k][2] = x1.x; raw[k][3] = x1.y;
+    }
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+        vv[0][t] = raw[0][t];
+        if constexpr (DERIV) {
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+                vv[1 + i][t] = g.Hinv[i * 3 + 0] * raw[1][t] + g.Hinv[i * 3 + 1] * raw[2][t] +
+                               g.Hinv[i * 3 + 2] * raw[3][t];
+        }
+    }
+#pragma unroll 1
+    for (int L = 0; L <= MAXLP; L++) {
+        const unsigned lo = max(it.lo, seg[L]), hi = min(it.hi, seg[L + 1]);
+        if (lo >= hi) continue;
+        switch (L) {
+            case 0: integ_segment<0, DERIV>(c, lo, hi, lane, vv, mom); break;
+            case 1: integ_segment<1, DERIV>(c, lo, hi, lane, vv, mom); break;
+            case 2: integ_segment<2, DERIV>(c, lo, hi, lane, vv, mom); break;
+            case 3: integ_segment<3, DERIV>(c, lo, hi, lane, vv, mom); break;
+            case 4: integ_segment<4, DERIV>(c, lo, hi, lane, vv, mom); break;
+            case 5: integ_segment<5, DERIV>(c, lo, hi, lane, vv, mom); break;
+            default: integ_segment<6, DERIV>(c, lo, hi, lane, vv, mom); break;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ FP64 peak probe
+// Register-only DFMA loop, 8 independent chains per thread: the denominator of the "alu" roofline.
+__global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, double seed) {
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+#pragma unroll 1
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int k = 0; k < 16; k++) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+    }
+    const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (s == 12345.678) out[0] = s;   // never true; keeps the chains alive
+}
+
+}  // namespace gpw
+
+// =============================================================================================== C ABI
+using namespace gpw;
+
+struct gpw_plan {
+    HostPlan *hp = nullptr;
+    bool on_device = false;
+    int device = -1;
+    long device_bytes = 0;
+    // device copies
+    TaskK *d_taskK = nullptr;
+    TaskP *d_taskP = nullptr;
+    Visit *d_visit = nullptr;
+    Item *d_item = nullptr;
+    double *d_S = nullptr;
+    long long *d_tile_base[GPW_MAX_LEVEL] = {nullptr};
+    unsigned *d_seg[GPW_MAX_LEVEL] = {nullptr};
+    double *d_coef = nullptr;   // polynomial workspace of gpw_eval_rho
+    double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
+};
+
+namespace {
+
+bool cuda_ok(cudaError_t e, const char *what) {
+    if (e == cudaSuccess) return true;
+    set_error(std::string(what) + ": " + cudaGetErrorString(e));
+    return false;
+}
+
+template <class T>
+bool upload(T **dst, const T *src, size_t n, long &bytes, const char *what) {
+    *dst = nullptr;
+    const size_t nb = sizeof(T) * (n ? n : 1);
+    if (!cuda_ok(cudaMalloc((void **)dst, nb), what)) return false;
+    bytes += (long)nb;
+    if (n && !cuda_ok(cudaMemcpy(*dst, src, sizeof(T) * n, cudaMemcpyHostToDevice), what)) return false;
+    return true;
+}
+
+void free_device(gpw_plan *p) {
+    cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_visit); cudaFree(p->d_item); cudaFree(p->d_S);
+    cudaFree(p->d_coef); cudaFree(p->d_mom);
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) { cudaFree(p->d_tile_base[a]); cudaFree(p->d_seg[a]); }
+}
+
+void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
+    std::memset(&P, 0, sizeof(P));
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++) {
+        P.lev[a] = hp->lev[a];
+        P.tile_base[a] = p->d_tile_base[a];
+        P.seg[a] = p->d_seg[a];
+        P.grid[a] = grids[a];
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *gpw_last_error(void) { return gpw::last_error_cstr(); }
+
+int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
+                    const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
+                    const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
+                    double tau, double rel_cutoff, int hermi, gpw_plan **plan_out) {
+    if (!plan_out) { set_error("gpw_build_pairs: plan_out is null"); return GPW_EINVAL; }
+    *plan_out = nullptr;
+    HostPlan *hp = nullptr;
+    const int rc = build_host_plan(cell, natm, xyz, nshl, shl_atom, shl_l, shl_nprim, shl_prim_off, prim_exp,
+                                   prim_coef, nlevel, mesh, tau, rel_cutoff, hermi, &hp);
+    if (rc != GPW_OK) return rc;
+    gpw_plan *p = new (std::nothrow) gpw_plan();
+    if (!p) { delete hp; set_error("out of host memory"); return GPW_ENOMEM; }
+    p->hp = hp;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();   // host-only plan: introspection works, eval calls fail with GPW_ECUDA
+        *plan_out = p;
+        return GPW_OK;
+    }
+    cudaGetDevice(&p->device);
+    bool ok = true;
+    long &nb = p->device_bytes;
+    ok = ok && upload(&p->d_taskK, hp->taskK.data(), hp->taskK.size(), nb, "upload pairs");
+    ok = ok && upload(&p->d_taskP, hp->taskP.data(), hp->taskP.size(), nb, "upload pairs");
+    ok = ok && upload(&p->d_visit, hp->visit.data(), hp->visit.size(), nb, "upload visit lists");
+    ok = ok && upload(&p->d_item, hp->item.data(), hp->item.size(), nb, "upload work items");
+    if (ok) {
+        std::vector<double> S_all((size_t)hp->nlevel * S_TOTAL);
+        for (int a = 0; a < hp->nlevel; a++) std::memcpy(S_all.data() + (size_t)a * S_TOTAL, hp->S[a].data(), sizeof(double) * S_TOTAL);
+        ok = upload(&p->d_S, S_all.data(), S_all.size(), nb, "upload monomial maps");
+    }
+    for (int a = 0; a < hp->nlevel && ok; a++) {
+        ok = ok && upload(&p->d_tile_base[a], hp->tile_base[a].data(), hp->tile_base[a].size(), nb, "upload block offsets");
+        ok = ok && upload(&p->d_seg[a], hp->seg[a].data(), hp->seg[a].size(), nb, "upload block segments");
+    }
+    const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
+    ok = ok && cuda_ok(cudaMalloc((void **)&p->d_coef, sizeof(double) * nw), "allocate polynomial workspace");
+    ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
+    if (ok) nb += (long)(2 * sizeof(double) * nw);
+    if (!ok) {
+        free_device(p);
+        delete hp;
+        delete p;
+        return GPW_ECUDA;
+    }
+    p->on_device = true;
+    *plan_out = p;
+    return GPW_OK;
+}
+
+void gpw_free_plan(gpw_plan *p) {
+    if (!p) return;
+    if (p->on_device) free_device(p);
+    delete p->hp;
+    delete p;
+}
+
+int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
+    if (!p || !out) { set_error("gpw_plan_info: null argument"); return GPW_EINVAL; }
+    const HostPlan *hp = p->hp;
+    std::memset(out, 0, sizeof(*out));
+    out->nao = hp->nao; out->nshl = hp->nshl; out->nlevel = hp->nlevel; out->hermi = hp->hermi;
+    out->on_device = p->on_device ? 1 : 0;
+    out->ntask = (long)hp->task.size();
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) {
+        out->ntask_level[a] = hp->ntask_level[a];
+        out->nvisit_level[a] = hp->nvisit_level[a];
+        for (int i = 0; i <= MAXL; i++)
+            for (int j = 0; j <= MAXL; j++) out->nvisit_class[a][i][j] = hp->nvisit_class[a][i][j];
+    }
+    out->nitem = (long)hp->item.size();
+    out->ncoef_total = (long)hp->ncoef_total;
+    out->build_seconds = hp->build_seconds;
+    out->device_bytes = p->device_bytes;
+    return GPW_OK;
+}
+
+int gpw_plan_export_tasks(const gpw_plan *p, gpw_task *buf, long cap, long *ntask) {
+    if (!p || !ntask) { set_error("gpw_plan_export_tasks: null argument"); return GPW_EINVAL; }
+    const HostPlan *hp = p->hp;
+    *ntask = (long)hp->task.size();
+    if (!buf) return GPW_OK;
+    const long n = std::min(cap, *ntask);
+    for (long i = 0; i < n; i++) {
+        const HostTask &t = hp->task[i];
+        gpw_task &o = buf[i];
+        o.shl_a = t.shl_a; o.prim_a = t.prim_a; o.shl_b = t.shl_b; o.prim_b = t.prim_b;
+        o.T[0] = t.T[0]; o.T[1] = t.T[1]; o.T[2] = t.T[2];
+        o.level = t.level; o.R = t.R;
+    }
+    return GPW_OK;
+}
+
+int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *const *rho_dev, void *cuda_stream) {
+    if (!p || !D_dev || !rho_dev) { set_error("gpw_eval_rho: null argument"); return GPW_EINVAL; }
+    if (deriv != 0 && deriv != 1) { set_error("gpw_eval_rho: deriv must be 0 or 1"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_rho: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++)
+        if (!rho_dev[a]) { set_error("gpw_eval_rho: null level pointer"); return GPW_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int ncomp = deriv ? 4 : 1;
+    for (int a = 0; a < hp->nlevel; a++) {
+        const LevelGeom &g = hp->lev[a];
+        const size_t nb = sizeof(double) * (size_t)g.N[0] * g.N[1] * g.N[2] * ncomp;
+        if (!cuda_ok(cudaMemsetAsync(rho_dev[a], 0, nb, st), "gpw_eval_rho: memset")) return GPW_ECUDA;
+    }
+    const int ntask = (int)hp->task.size(), nitem = (int)hp->item.size();
+    if (ntask == 0 || nitem == 0) return GPW_OK;
+    k_poly_from_D<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, D_dev, hp->nao, p->d_S, p->d_coef);
+    GridParams P;
+    fill_params(p, P, rho_dev);
+    const int nblk = (nitem + 3) / 4;
+    if (deriv) k_collocate<1><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef);
+    else k_collocate<0><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef);
+    if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
+    return GPW_OK;
+}
+
+int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, double *F_dev, void *cuda_stream) {
+    if (!p || !v_dev || !F_dev) { set_error("gpw_eval_mat: null argument"); return GPW_EINVAL; }
+    if (deriv != 0 && deriv != 1) { set_error("gpw_eval_mat: deriv must be 0 or 1"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_mat: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++)
+        if (!v_dev[a]) { set_error("gpw_eval_mat: null level pointer"); return GPW_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
+    const int ntask = (int)hp->task.size(), nitem = (int)hp->item.size();
+    if (ntask == 0 || nitem == 0) return GPW_OK;
+    if (!cuda_ok(cudaMemsetAsync(p->d_mom, 0, sizeof(double) * (size_t)hp->ncoef_total, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
+    GridParams P;
+    fill_params(p, P, const_cast<double *const *>(v_dev));
+    const int nblk = (nitem + 3) / 4;
+    if (deriv) k_integrate<1><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_mom);
+    else k_integrate<0><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_mom);
+    DVs dv;
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) dv.v[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;
+    k_F_from_moments<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, p->d_mom, p->d_S, dv, F_dev, hp->nao);
+    if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat: kernel launch")) return GPW_ECUDA;
+    return GPW_OK;
+}
+
+int gpw_dfma_peak(double min_seconds, double *tflops_out, int *sm_count_out) {
+    if (!tflops_out) { set_error("gpw_dfma_peak: null argument"); return GPW_EINVAL; }
+    int dev = 0, nsm = 0;
+    if (!cuda_ok(cudaGetDevice(&dev), "gpw_dfma_peak") ||
+        !cuda_ok(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "gpw_dfma_peak")) return GPW_ECUDA;
+    if (sm_count_out) *sm_count_out = nsm;
+    double *d = nullptr;
+    if (!cuda_ok(cudaMalloc((void **)&d, 8), "gpw_dfma_peak")) return GPW_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = nsm * 8, threads = 256;
+    int iters = 2048;
+    double best = 0.0, spent = 0.0;
+    k_dfma_peak<<<blocks, threads>>>(d, 64, 1.0);   // warm-up
+    while (spent < min_seconds || best == 0.0) {
+        cudaEventRecord(e0);
+        k_dfma_peak<<<blocks, threads>>>(d, iters, 1.0);
+        cudaEventRecord(e1);
+        if (!cuda_ok(cudaEventSynchronize(e1), "gpw_dfma_peak")) { cudaFree(d); return GPW_ECUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * 8 * 16 * (double)iters * blocks * threads;
+        best = std::max(best, flops / (ms * 1e-3) / 1e12);
+        spent += ms * 1e-3;
+        if (ms < 20.0f) iters *= 2;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    *tflops_out = best;
+    return GPW_OK;
+}
+
+int gpw_interp_up(gpw_plan *, const double *const *, int, double *, void *) {
+    set_error("gpw_interp_up: not built yet");
+    return GPW_EUNSUPPORTED;
+}
+int gpw_restrict_down(gpw_plan *, const double *, int, double *const *, void *) {
+    set_error("gpw_restrict_down: not built yet");
+    return GPW_EUNSUPPORTED;
+}
+
+}  // extern "C"

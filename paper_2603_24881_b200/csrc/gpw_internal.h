@@ -1,0 +1,128 @@
+// Internal structures shared by the host plan builder (plan.cpp) and the CUDA side (*.cu).
+// Not part of the C ABI (include/gpw.h is).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "gpw.h"
+
+#if defined(__CUDACC__)
+#define GPW_CX __host__ __device__ constexpr
+#else
+#define GPW_CX constexpr
+#endif
+
+namespace gpw {
+
+constexpr int MAXL = GPW_MAX_L;          // shells up to f
+constexpr int MAXLP = 2 * MAXL;          // pair polynomial degree L = la + lb <= 6
+constexpr int NLSEG = MAXLP + 1;         // visit lists are segmented by L = 0..6
+constexpr int TILE = 4;                  // grid block edge
+
+// number of monomials u1^kx u2^ky u3^kz with kx+ky+kz <= L
+GPW_CX int ncoef(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
+// per-pair workspace stride (kept even so that rows stay 16-byte aligned)
+GPW_CX int ncoef_pad(int L) { return (ncoef(L) + 1) & ~1; }
+GPW_CX int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+
+// Geometry of one multigrid level (plain data: copied to the device as is).
+struct LevelGeom {
+    int N[3];        // mesh
+    int T[3];        // 4x4x4 blocks per axis
+    int ntile;       // T[0]*T[1]*T[2]
+    int pad0;
+    double H[9];     // H[c*3+i] = component c of the grid step vector a_i / N_i :  r - P = H (n - n_P)
+    double Hinv[9];  // Hinv[i*3+c]:  u_i = sum_c Hinv[i*3+c] X_c
+    double Gm[6];    // H^T H, packed 11 22 33 12 13 23 : |H u|^2 = u^T Gm u
+    double dV;       // Omega / (N1 N2 N3)   (Eq. 29)
+    double ecut;     // E_alpha of T5
+};
+
+// Pair record read by the collocation / integration kernels (48 bytes, three 16-byte loads).
+struct TaskK {
+    double nP[3];        // Gaussian-product centre P in grid-index units of its level
+    double ap;           // a_p = a_a + a_b
+    double cc;           // exp(-2 a_p Gm33): second-order ratio of the Gaussian recursion along n3 (Eq. 25)
+    long long coef_off;  // offset (doubles) of the pair's polynomial / moment vector in the workspace
+};
+static_assert(sizeof(TaskK) == 48, "TaskK must be 48 bytes");
+
+// Pair record read by the pre-pass (D block -> polynomial) and post-pass (moments -> F block).
+struct TaskP {
+    double PA[3];    // P - A
+    double PB[3];    // P - (B + T)
+    double pref;     // coef_a coef_b exp(-a_a a_b / a_p |A - B - T|^2)
+    long long coef_off;
+    int ao_a, ao_b;
+    short la, lb;
+    short level;
+    short sym;       // 1: use D_ab + D_ba and mirror F (hermi, not the a==b,T==0 pair)
+};
+
+// One (pair, 4x4x4 block) visit in a block's list.
+struct Visit {
+    int task;             // global pair index
+    signed char s[3];     // lattice wraps: unwrapped block = stored block + s * T
+    unsigned char pad;
+};
+static_assert(sizeof(Visit) == 8, "Visit must be 8 bytes");
+
+// Work item of the grid kernels: a contiguous range of one block's visit list.
+struct Item {
+    int level;
+    int tile;             // stored block index on its level
+    unsigned lo, hi;      // visit range relative to the block's list
+    int single;           // 1: the only item of its block (plain store), 0: accumulate atomically
+    int pad;
+};
+
+struct HostTask {
+    int shl_a, prim_a, shl_b, prim_b;
+    int T[3];
+    int level, la, lb;
+    double R, ap, pref;
+    double P[3], A[3], Bt[3];
+    int sym;
+};
+
+struct HostPlan {
+    // inputs kept
+    double cell[9], binv[9], bnorm[3], omega;
+    int natm = 0, nshl = 0, nprim = 0, nlevel = 0, nao = 0, hermi = 0;
+    double tau = 0, rel_cutoff = 0;
+    std::vector<int> ao_loc;
+    std::vector<LevelGeom> lev;
+    std::vector<std::vector<double>> S;   // per level: Cartesian -> grid-index monomial maps, degree blocks
+    std::vector<HostTask> task;           // sorted by (level, L, enumeration order)
+    std::vector<TaskK> taskK;
+    std::vector<TaskP> taskP;
+    long long ncoef_total = 0;
+    // per level block lists
+    std::vector<std::vector<long long>> tile_base;   // [level][ntile+1] global visit index
+    std::vector<std::vector<unsigned>> seg;          // [level][ntile*8] start of each L segment (relative)
+    std::vector<Visit> visit;                        // all levels, level-major, block-major
+    std::vector<Item> item;                          // sorted by descending size
+    long nvisit_level[GPW_MAX_LEVEL] = {0};
+    long ntask_level[GPW_MAX_LEVEL] = {0};
+    long nvisit_class[GPW_MAX_LEVEL][MAXL + 1][MAXL + 1] = {{{0}}};
+    double build_seconds = 0;
+};
+
+// offsets of the degree blocks inside S[level]: block d is n_d x n_d, n_d = (d+1)(d+2)/2
+GPW_CX int s_block_off(int d) {
+    int o = 0;
+    for (int e = 0; e < d; e++) { int n = (e + 1) * (e + 2) / 2; o += n * n; }
+    return o;
+}
+constexpr int S_TOTAL = 1 + 9 + 36 + 100 + 225 + 441 + 784;
+
+void set_error(const std::string &msg);
+
+// plan.cpp
+int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
+                    const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
+                    const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
+                    double tau, double rel_cutoff, int hermi, HostPlan **out);
+
+}  // namespace gpw

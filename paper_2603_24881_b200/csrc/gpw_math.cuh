@@ -1,0 +1,268 @@
+// Per-thread arithmetic of the collocation / integration path, written as __host__ __device__
+// templates so that the identical code can be stepped on the host while developing.
+//
+// Formulation:  for one primitive pair the product of Eq. (23) is
+//     sum_ij D_ij phi_a,i(r) phi_b,j(r - T) = Q(r - P) exp(-a_p |r - P|^2)
+// with Q a polynomial of total degree L = la + lb.  A pre-pass expands Q about the Gaussian-product
+// centre P (binomial expansion, Eq. 26-27) and rewrites it in grid-index coordinates
+// u = n - n_P (r - P = H u, H = grid step matrix), which keeps one code path for orthorhombic and
+// non-orthogonal cells (the paper's A.30-A.33 split).  A thread owns a column of four
+// grid points along n3: stage A collapses the polynomial to a[kz](u1,u2), stage B is a Horner sweep in
+// u3.  The Gaussian along the column follows the recursion of Eq. (24)-(25).
+// Integration is the exact transpose: column moments, then outer products into the pair's moment vector.
+#pragma once
+#include "gpw_internal.h"
+
+#if defined(__CUDACC__)
+#define GPW_HD __host__ __device__ __forceinline__
+#else
+#define GPW_HD inline
+#endif
+
+namespace gpw {
+
+// position of u1^kx u2^ky u3^kz in a pair's polynomial of degree L (kz-major, then ky, then kx)
+GPW_HD constexpr int cidx(int L, int kx, int ky, int kz) {
+    int o = 0;
+    for (int z = 0; z < kz; z++) o += (L - z + 1) * (L - z + 2) / 2;
+    for (int y = 0; y < ky; y++) o += (L - kz - y + 1);
+    return o + kx;
+}
+// position of a degree-d monomial X^a Y^b Z^c in the degree-graded order (degree blocks, inside a block
+// decreasing a then decreasing b)
+GPW_HD constexpr int gidx(int a, int b, int c) {
+    const int d = a + b + c;
+    const int r = d - a;
+    return d * (d + 1) * (d + 2) / 6 + r * (r + 1) / 2 + (r - b);
+}
+
+GPW_HD void cart_of(int l, int i, int &lx, int &ly, int &lz) {
+    // component i of a shell: decreasing lx, then decreasing ly
+    int n = 0;
+    for (int x = l; x >= 0; x--)
+        for (int y = l - x; y >= 0; y--) {
+            if (n == i) { lx = x; ly = y; lz = l - x - y; return; }
+            n++;
+        }
+    lx = ly = lz = 0;
+}
+
+// 1-D binomial tables: Tt[x][i][j][k] = coefficient of X^k in (X + PA_x)^i (X + PB_x)^j   (Eq. 26-27)
+struct BinomTables {
+    double t[3][MAXL + 1][MAXL + 1][MAXLP + 1];
+};
+
+GPW_HD void build_binom(const TaskP &p, BinomTables &B) {
+    const int la = p.la, lb = p.lb;
+    for (int x = 0; x < 3; x++) {
+        for (int i = 0; i <= la; i++)
+            for (int j = 0; j <= lb; j++) {
+                double *cur = B.t[x][i][j];
+                for (int k = 0; k <= MAXLP; k++) cur[k] = 0.0;
+                if (i == 0 && j == 0) { cur[0] = 1.0; continue; }
+                const double *prev = i > 0 ? B.t[x][i - 1][j] : B.t[x][i][j - 1];
+                const double off = i > 0 ? p.PA[x] : p.PB[x];
+                for (int k = 0; k <= i + j; k++) cur[k] = (k > 0 ? prev[k - 1] : 0.0) + off * prev[k];
+            }
+    }
+}
+
+// Pre-pass: polynomial of one pair from its block of the density matrix.
+//   out[cidx(L, k)] = pref * sum_ij Dsym_ij [coefficient of u^k in (r-A)^i (r-B-T)^j]
+// S: this level's Cartesian -> grid-index monomial maps (degree blocks).
+GPW_HD void pair_poly_from_D(const TaskP &p, const double *D, int nao, const double *S, double *out) {
+    const int la = p.la, lb = p.lb, L = la + lb;
+    BinomTables B;
+    build_binom(p, B);
+    double Cg[ncoef(MAXLP)];
+    const int nc = ncoef(L);
+    for (int k = 0; k < nc; k++) Cg[k] = 0.0;
+    const int nca = ncart(la), ncb = ncart(lb);
+    for (int i = 0; i < nca; i++) {
+        int ix, iy, iz;
+        cart_of(la, i, ix, iy, iz);
+        for (int j = 0; j < ncb; j++) {
+            int jx, jy, jz;
+            cart_of(lb, j, jx, jy, jz);
+            double d = D[(long long)(p.ao_a + i) * nao + p.ao_b + j];
+            if (p.sym) d += D[(long long)(p.ao_b + j) * nao + p.ao_a + i];
+            for (int kx = 0; kx <= ix + jx; kx++) {
+                const double tx = d * B.t[0][ix][jx][kx];
+                for (int ky = 0; ky <= iy + jy; ky++) {
+                    const double txy = tx * B.t[1][iy][jy][ky];
+                    for (int kz = 0; kz <= iz + jz; kz++) Cg[gidx(kx, ky, kz)] += txy * B.t[2][iz][jz][kz];
+                }
+            }
+        }
+    }
+    // Cartesian -> grid-index coordinates, degree by degree, into the Horner order
+    for (int d = 0; d <= L; d++) {
+        const int nd = (d + 1) * (d + 2) / 2;
+        const double *Sd = S + s_block_off(d);
+        const double *Cd = Cg + d * (d + 1) * (d + 2) / 6;
+        int row = 0;
+        for (int a = d; a >= 0; a--)
+            for (int b = d - a; b >= 0; b--, row++) {
+                double s = 0.0;
+                for (int col = 0; col < nd; col++) s += Sd[row * nd + col] * Cd[col];
+                out[cidx(L, a, b, d - a - b)] = p.pref * s;
+            }
+    }
+}
+
+// Post-pass: F block of one pair from its moment vector  m[cidx(L,k)] = sum_r w(r) G(r) u^k.
+//   Fblk[i*ncb + j] = pref * dV * sum_k [coefficient of u^k in (r-A)^i (r-B-T)^j] m[k]
+GPW_HD void pair_block_from_moments(const TaskP &p, const double *m, const double *S, double dV, double *Fblk) {
+    const int la = p.la, lb = p.lb, L = la + lb;
+    BinomTables B;
+    build_binom(p, B);
+    double Cg[ncoef(MAXLP)];
+    for (int d = 0; d <= L; d++) {
+        const int nd = (d + 1) * (d + 2) / 2;
+        const double *Sd = S + s_block_off(d);
+        double *Cd = Cg + d * (d + 1) * (d + 2) / 6;
+        for (int col = 0; col < nd; col++) Cd[col] = 0.0;
+        int row = 0;
+        for (int a = d; a >= 0; a--)
+            for (int b = d - a; b >= 0; b--, row++) {
+                const double mv = m[cidx(L, a, b, d - a - b)];
+                for (int col = 0; col < nd; col++) Cd[col] += Sd[row * nd + col] * mv;
+            }
+    }
+    const int nca = ncart(la), ncb = ncart(lb);
+    const double scale = p.pref * dV;
+    for (int i = 0; i < nca; i++) {
+        int ix, iy, iz;
+        cart_of(la, i, ix, iy, iz);
+        for (int j = 0; j < ncb; j++) {
+            int jx, jy, jz;
+            cart_of(lb, j, jx, jy, jz);
+            double s = 0.0;
+            for (int kx = 0; kx <= ix + jx; kx++)
+                for (int ky = 0; ky <= iy + jy; ky++) {
+                    const double txy = B.t[0][ix][jx][kx] * B.t[1][iy][jy][ky];
+                    for (int kz = 0; kz <= iz + jz; kz++) s += txy * B.t[2][iz][jz][kz] * Cg[gidx(kx, ky, kz)];
+                }
+            Fblk[i * ncb + j] = scale * s;
+        }
+    }
+}
+
+// Gaussian exp(-a_p |H u|^2) on the four points u3 = u30 + t of a column, by the two-term recursion of
+// Eq. (24)-(25) generalised to a non-orthogonal step matrix (cross terms of A.30-A.33 enter through the
+// slope).  q[6] = a_p * Gm (11 22 33 12 13 23), cc = exp(-2 q33).
+GPW_HD void column_gauss(const double *q, double cc, double u1, double u2, double u30, double *G) {
+    const double E0 = q[0] * u1 * u1 + q[1] * u2 * u2 + q[2] * u30 * u30 +
+                      2.0 * (q[3] * u1 * u2 + (q[4] * u1 + q[5] * u2) * u30);
+    const double sl = 2.0 * (q[4] * u1 + q[5] * u2 + q[2] * u30) + q[2];
+    double g = exp(-E0);
+    double r = exp(-sl);
+    G[0] = g;
+    g *= r; r *= cc; G[1] = g;
+    g *= r; r *= cc; G[2] = g;
+    g *= r; G[3] = g;
+}
+
+// Collocation of one pair on one column of four points.
+//   c      the pair's polynomial (cidx order), broadcast reads
+//   acc    [NCOMP][4] running sums; for DERIV the gradient is accumulated in grid-index coordinates
+//          (the constant map to Cartesian is applied once when the block is written)
+template <int L, int DERIV>
+GPW_HD void colloc_column(const double *__restrict__ c, const double *q, double cc, double u1, double u2,
+                          double u30, double (*acc)[4]) {
+    double a[L + 1], ax[L + 1], ay[L + 1];
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++) {
+        double s = 0.0, sx = 0.0, sy = 0.0;
+#pragma unroll
+        for (int ky = L - kz; ky >= 0; ky--) {
+            double p = 0.0, dp = 0.0;
+#pragma unroll
+            for (int kx = L - kz - ky; kx >= 0; kx--) {
+                if (DERIV) dp = dp * u1 + p;
+                p = p * u1 + c[cidx(L, kx, ky, kz)];
+            }
+            if (DERIV) { sy = sy * u2 + s; sx = sx * u2 + dp; }
+            s = s * u2 + p;
+        }
+        a[kz] = s; ax[kz] = sx; ay[kz] = sy;
+    }
+    double G[4];
+    column_gauss(q, cc, u1, u2, u30, G);
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+        const double u3 = u30 + t;
+        double Q = 0.0, Qz = 0.0, Qx = 0.0, Qy = 0.0;
+#pragma unroll
+        for (int kz = L; kz >= 0; kz--) {
+            if (DERIV) { Qz = Qz * u3 + Q; Qx = Qx * u3 + ax[kz]; Qy = Qy * u3 + ay[kz]; }
+            Q = Q * u3 + a[kz];
+        }
+        acc[0][t] += G[t] * Q;
+        if constexpr (DERIV != 0) {
+            const double m2Q = -2.0 * Q;
+            const double qu1 = q[0] * u1 + q[3] * u2 + q[4] * u3;
+            const double qu2 = q[3] * u1 + q[1] * u2 + q[5] * u3;
+            const double qu3 = q[4] * u1 + q[5] * u2 + q[2] * u3;
+            acc[1][t] += G[t] * (Qx + m2Q * qu1);
+            acc[2][t] += G[t] * (Qy + m2Q * qu2);
+            acc[3][t] += G[t] * (Qz + m2Q * qu3);
+        }
+    }
+}
+
+// Integration of one pair on one column of four points (transpose of colloc_column).
+//   v      [NCOMP][4]: v0 and, for DERIV, the vector field already mapped to grid-index coordinates
+//   m      the thread's private moment vector (cidx order), accumulated
+template <int L, int DERIV>
+GPW_HD void integ_column(const double (*v)[4], const double *q, double cc, double u1, double u2, double u30,
+                         double *m) {
+    double G[4];
+    column_gauss(q, cc, u1, u2, u30, G);
+    double A0[L + 1], A1[L + 1], A2[L + 1], A3[L + 1];
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++) { A0[kz] = 0.0; A1[kz] = 0.0; A2[kz] = 0.0; A3[kz] = 0.0; }
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+        const double u3 = u30 + t;
+        double g0 = v[0][t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
+        if constexpr (DERIV != 0) {
+            const double qu1 = q[0] * u1 + q[3] * u2 + q[4] * u3;
+            const double qu2 = q[3] * u1 + q[1] * u2 + q[5] * u3;
+            const double qu3 = q[4] * u1 + q[5] * u2 + q[2] * u3;
+            g0 -= 2.0 * (v[1][t] * qu1 + v[2][t] * qu2 + v[3][t] * qu3);
+            g1 = G[t] * v[1][t]; g2 = G[t] * v[2][t]; g3 = G[t] * v[3][t];
+        }
+        g0 *= G[t];
+        double pw = 1.0;
+#pragma unroll
+        for (int kz = 0; kz <= L; kz++) {
+            A0[kz] += g0 * pw;
+            if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
+            pw *= u3;
+        }
+    }
+    if (DERIV) {
+#pragma unroll
+        for (int kz = 1; kz <= L; kz++) A0[kz] += kz * A3[kz - 1];
+    }
+    double p1[L + 1], p2[L + 1];
+    p1[0] = 1.0; p2[0] = 1.0;
+#pragma unroll
+    for (int k = 1; k <= L; k++) { p1[k] = p1[k - 1] * u1; p2[k] = p2[k - 1] * u2; }
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+        for (int ky = 0; ky <= L - kz; ky++)
+#pragma unroll
+            for (int kx = 0; kx <= L - kz - ky; kx++) {
+                double s = A0[kz] * (p1[kx] * p2[ky]);
+                if (DERIV) {
+                    if (kx > 0) s += A1[kz] * (kx * (p1[kx - 1] * p2[ky]));
+                    if (ky > 0) s += A2[kz] * (ky * (p1[kx] * p2[ky - 1]));
+                }
+                m[cidx(L, kx, ky, kz)] += s;
+            }
+}
+
+}  // namespace gpw

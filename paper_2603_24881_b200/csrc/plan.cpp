@@ -1,0 +1,465 @@
+// Host side of gpw_build_pairs: cutoff radii, pair screening, lattice images, level assignment and
+// per-block visit lists.  Follows DESIGN.md T1..T6 (readings of PAPER.md:59, :123-138, :162-164, :200,
+// Alg. 4-5 at :435-561).  Plain C++17 + std::thread; no code shared with oracle/.
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <thread>
+
+#include "gpw_internal.h"
+
+namespace gpw {
+
+static thread_local std::string g_err;
+void set_error(const std::string &msg) { g_err = msg; }
+const char *last_error_cstr() { return g_err.c_str(); }
+
+namespace {
+
+inline int floordiv(int n, int d) { return n >= 0 ? n / d : -((-n + d - 1) / d); }
+inline int posmod(int n, int d) { int m = n % d; return m < 0 ? m + d : m; }
+
+// T1 (Eq. 20): largest root of r^2 |coef| r^l exp(-a r^2) = tau, 40 fixed-point steps.
+double prim_radius(int l, double a, double coef, double tau) {
+    const double C = std::log(std::fabs(coef)) - std::log(tau);
+    double r = std::sqrt(std::max(C, 1.0) / a) + 5.0;
+    for (int it = 0; it < 40; it++) {
+        const double arg = (C + (l + 2) * std::log(r)) / a;
+        if (arg <= 0.0) return 0.0;
+        r = std::sqrt(arg);
+    }
+    return r;
+}
+
+// T4: largest root of r^2 kappa (r+dA)^la (r+dB)^lb exp(-a_p r^2) = tau.
+double pair_radius(int la, int lb, double ap, double kappa, double dA, double dB, double tau) {
+    const double C = std::log(kappa) - std::log(tau);
+    double r = std::sqrt(std::max(C, 1.0) / ap) + dA + dB + 5.0;
+    for (int it = 0; it < 40; it++) {
+        const double arg = (C + 2.0 * std::log(r) + la * std::log(r + dA) + lb * std::log(r + dB)) / ap;
+        if (arg <= 0.0) return 0.0;
+        r = std::sqrt(arg);
+    }
+    return r;
+}
+
+bool invert3(const double *m, double *inv, double *det_out) {
+    const double det = m[0] * (m[4] * m[8] - m[5] * m[7]) - m[1] * (m[3] * m[8] - m[5] * m[6]) +
+                       m[2] * (m[3] * m[7] - m[4] * m[6]);
+    *det_out = det;
+    if (std::fabs(det) < 1e-12) return false;
+    inv[0] = (m[4] * m[8] - m[5] * m[7]) / det;
+    inv[1] = (m[2] * m[7] - m[1] * m[8]) / det;
+    inv[2] = (m[1] * m[5] - m[2] * m[4]) / det;
+    inv[3] = (m[5] * m[6] - m[3] * m[8]) / det;
+    inv[4] = (m[0] * m[8] - m[2] * m[6]) / det;
+    inv[5] = (m[2] * m[3] - m[0] * m[5]) / det;
+    inv[6] = (m[3] * m[7] - m[4] * m[6]) / det;
+    inv[7] = (m[1] * m[6] - m[0] * m[7]) / det;
+    inv[8] = (m[0] * m[4] - m[1] * m[3]) / det;
+    return true;
+}
+
+// index of monomial (a,b,c), a+b+c = d, inside its degree block: decreasing a, then decreasing b
+inline int graded_idx(int a, int b, int d) {
+    const int r = d - a;  // number of rows before: sum_{a'>a} (d-a'+1)
+    return r * (r + 1) / 2 + (r - b);
+}
+
+// S_d[row (p,q,r)][col (a,b,c)] = coefficient of u1^p u2^q u3^r in (H0.u)^a (H1.u)^b (H2.u)^c
+void build_S(const double *H, std::vector<double> &S) {
+    S.assign(S_TOTAL, 0.0);
+    for (int d = 0; d <= MAXLP; d++) {
+        const int nd = (d + 1) * (d + 2) / 2;
+        double *blk = S.data() + s_block_off(d);
+        for (int a = d; a >= 0; a--)
+            for (int b = d - a; b >= 0; b--) {
+                const int c = d - a - b;
+                const int col = graded_idx(a, b, d);
+                double poly[MAXLP + 1][MAXLP + 1][MAXLP + 1];
+                std::memset(poly, 0, sizeof(poly));
+                poly[0][0][0] = 1.0;
+                int deg = 0;
+                const int reps[3] = {a, b, c};
+                for (int x = 0; x < 3; x++)
+                    for (int rep = 0; rep < reps[x]; rep++) {
+                        double nxt[MAXLP + 1][MAXLP + 1][MAXLP + 1];
+                        std::memset(nxt, 0, sizeof(nxt));
+                        for (int p = 0; p <= deg; p++)
+                            for (int q = 0; q <= deg - p; q++) {
+                                const int r = deg - p - q;
+                                const double v = poly[p][q][r];
+                                if (v == 0.0) continue;
+                                nxt[p + 1][q][r] += v * H[x * 3 + 0];
+                                nxt[p][q + 1][r] += v * H[x * 3 + 1];
+                                nxt[p][q][r + 1] += v * H[x * 3 + 2];
+                            }
+                        std::memcpy(poly, nxt, sizeof(poly));
+                        deg++;
+                    }
+                for (int p = d; p >= 0; p--)
+                    for (int q = d - p; q >= 0; q--)
+                        blk[graded_idx(p, q, d) * nd + col] = poly[p][q][d - p - q];
+            }
+    }
+}
+
+struct RawVisit {
+    long long key;  // global block id (level-major)
+    int task;
+    signed char s[3];
+    unsigned char L;
+};
+
+template <class F>
+void parallel_chunks(long n, long chunk, int nthread, F &&fn) {
+    std::atomic<long> next(0);
+    auto worker = [&](int tid) {
+        for (;;) {
+            const long c = next.fetch_add(1);
+            const long lo = c * chunk;
+            if (lo >= n) break;
+            fn(c, lo, std::min(n, lo + chunk), tid);
+        }
+    };
+    std::vector<std::thread> th;
+    for (int t = 1; t < nthread; t++) th.emplace_back(worker, t);
+    worker(0);
+    for (auto &t : th) t.join();
+}
+
+}  // namespace
+
+int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
+                    const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
+                    const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
+                    double tau, double rel_cutoff, int hermi, HostPlan **out) {
+    const auto t_start = std::chrono::steady_clock::now();
+    if (!cell || !xyz || !shl_atom || !shl_l || !shl_nprim || !shl_prim_off || !prim_exp || !prim_coef ||
+        !mesh || !out) { set_error("gpw_build_pairs: null pointer argument"); return GPW_EINVAL; }
+    if (natm < 1 || nshl < 1) { set_error("gpw_build_pairs: natm and nshl must be >= 1"); return GPW_EINVAL; }
+    if (nlevel < 1 || nlevel > GPW_MAX_LEVEL) { set_error("gpw_build_pairs: nlevel must be in 1..8"); return GPW_EINVAL; }
+    if (!(tau > 0.0) || !(rel_cutoff > 0.0)) { set_error("gpw_build_pairs: tau and rel_cutoff must be > 0"); return GPW_EINVAL; }
+    if (hermi != 0 && hermi != 1) { set_error("gpw_build_pairs: hermi must be 0 or 1"); return GPW_EINVAL; }
+    for (int i = 0; i < 3 * nlevel; i++)
+        if (mesh[i] < 4 || mesh[i] % 4) { set_error("gpw_build_pairs: every mesh entry must be a positive multiple of 4"); return GPW_EINVAL; }
+    int nprim = 0;
+    for (int s = 0; s < nshl; s++) {
+        if (shl_l[s] < 0) { set_error("gpw_build_pairs: negative angular momentum"); return GPW_EINVAL; }
+        if (shl_l[s] > MAXL) { set_error("gpw_build_pairs: shells beyond f (l >= 4) are not supported"); return GPW_EUNSUPPORTED; }
+        if (shl_atom[s] < 0 || shl_atom[s] >= natm) { set_error("gpw_build_pairs: shl_atom out of range"); return GPW_EINVAL; }
+        if (shl_nprim[s] < 1 || shl_prim_off[s] < 0) { set_error("gpw_build_pairs: shl_nprim must be >= 1 and offsets >= 0"); return GPW_EINVAL; }
+        nprim = std::max(nprim, shl_prim_off[s] + shl_nprim[s]);
+    }
+    for (int s = 0; s < nshl; s++)
+        for (int k = 0; k < shl_nprim[s]; k++)
+            if (!(prim_exp[shl_prim_off[s] + k] > 0.0)) { set_error("gpw_build_pairs: primitive exponents must be > 0"); return GPW_EINVAL; }
+
+    HostPlan *hp = new (std::nothrow) HostPlan();
+    if (!hp) { set_error("out of host memory"); return GPW_ENOMEM; }
+    try {
+        std::memcpy(hp->cell, cell, sizeof(double) * 9);
+        double det;
+        if (!invert3(cell, hp->binv, &det)) { delete hp; set_error("gpw_build_pairs: singular cell (|det| < 1e-12)"); return GPW_EINVAL; }
+        hp->omega = std::fabs(det);
+        // binv[c*3+i] = component c of b_i, so that u_i = sum_c r_c binv[c*3+i]
+        for (int i = 0; i < 3; i++)
+            hp->bnorm[i] = std::sqrt(hp->binv[0 * 3 + i] * hp->binv[0 * 3 + i] + hp->binv[1 * 3 + i] * hp->binv[1 * 3 + i] +
+                                     hp->binv[2 * 3 + i] * hp->binv[2 * 3 + i]);
+        hp->natm = natm; hp->nshl = nshl; hp->nprim = nprim; hp->nlevel = nlevel; hp->hermi = hermi;
+        hp->tau = tau; hp->rel_cutoff = rel_cutoff;
+        hp->ao_loc.resize(nshl + 1);
+        hp->ao_loc[0] = 0;
+        for (int s = 0; s < nshl; s++) hp->ao_loc[s + 1] = hp->ao_loc[s] + ncart(shl_l[s]);
+        hp->nao = hp->ao_loc[nshl];
+
+        // ---- level geometry (T5: E_alpha = 0.5 min_i (pi N_i |b_i|)^2) ----
+        hp->lev.resize(nlevel);
+        hp->S.resize(nlevel);
+        for (int a = 0; a < nlevel; a++) {
+            LevelGeom &g = hp->lev[a];
+            std::memset(&g, 0, sizeof(g));
+            double e = 1e300;
+            for (int i = 0; i < 3; i++) {
+                g.N[i] = mesh[a * 3 + i];
+                g.T[i] = g.N[i] / TILE;
+                const double gg = M_PI * g.N[i] * hp->bnorm[i];
+                e = std::min(e, 0.5 * gg * gg);
+            }
+            g.ecut = e;
+            g.ntile = g.T[0] * g.T[1] * g.T[2];
+            g.dV = hp->omega / ((double)g.N[0] * g.N[1] * g.N[2]);
+            for (int c = 0; c < 3; c++)
+                for (int i = 0; i < 3; i++) {
+                    g.H[c * 3 + i] = cell[i * 3 + c] / g.N[i];
+                    g.Hinv[i * 3 + c] = hp->binv[c * 3 + i] * g.N[i];
+                }
+            const int pr[6][2] = {{0, 0}, {1, 1}, {2, 2}, {0, 1}, {0, 2}, {1, 2}};
+            for (int k = 0; k < 6; k++) {
+                double s = 0;
+                for (int c = 0; c < 3; c++) s += g.H[c * 3 + pr[k][0]] * g.H[c * 3 + pr[k][1]];
+                g.Gm[k] = s;
+            }
+            build_S(g.H, hp->S[a]);
+        }
+
+        // ---- T1 radii ----
+        std::vector<double> prad(nprim, 0.0);
+        std::vector<int> prim_shl(nprim, -1);
+        for (int s = 0; s < nshl; s++)
+            for (int k = 0; k < shl_nprim[s]; k++) {
+                const int p = shl_prim_off[s] + k;
+                prad[p] = prim_radius(shl_l[s], prim_exp[p], prim_coef[p], tau);
+                prim_shl[p] = s;
+            }
+
+        // ---- T2..T5: enumerate pairs (a, b, T), parallel over shell a ----
+        int nthread = (int)std::thread::hardware_concurrency();
+        if (nthread < 1) nthread = 1;
+        if (nthread > 64) nthread = 64;
+        std::vector<std::vector<HostTask>> per_shell(nshl);
+        parallel_chunks(nshl, 1, nthread, [&](long, long lo, long hi, int) {
+            for (long sa = lo; sa < hi; sa++) {
+                std::vector<HostTask> &outv = per_shell[sa];
+                for (int sb = 0; sb < nshl; sb++)
+                    for (int ka = 0; ka < shl_nprim[sa]; ka++)
+                        for (int kb = 0; kb < shl_nprim[sb]; kb++) {
+                            const int pa = shl_prim_off[sa] + ka, pb = shl_prim_off[sb] + kb;
+                            if (hermi && pa < pb) continue;  // canonical unordered set (A14)
+                            const double ra = prad[pa], rb = prad[pb];
+                            if (ra <= 0.0 || rb <= 0.0) continue;
+                            const double *A = xyz + 3 * shl_atom[sa], *B = xyz + 3 * shl_atom[sb];
+                            const double rsum = ra + rb;
+                            const double d[3] = {A[0] - B[0], A[1] - B[1], A[2] - B[2]};
+                            int tlo[3], thi[3];
+                            for (int i = 0; i < 3; i++) {
+                                const double f = d[0] * hp->binv[0 * 3 + i] + d[1] * hp->binv[1 * 3 + i] + d[2] * hp->binv[2 * 3 + i];
+                                const double w = rsum * hp->bnorm[i];
+                                tlo[i] = (int)std::ceil(f - w);
+                                thi[i] = (int)std::floor(f + w);
+                            }
+                            for (int t0 = tlo[0]; t0 <= thi[0]; t0++)
+                                for (int t1 = tlo[1]; t1 <= thi[1]; t1++)
+                                    for (int t2 = tlo[2]; t2 <= thi[2]; t2++) {
+                                        if (hermi && pa == pb) {  // keep T = 0 or T lexicographically positive
+                                            if (t0 < 0 || (t0 == 0 && (t1 < 0 || (t1 == 0 && t2 < 0)))) continue;
+                                        }
+                                        HostTask t;
+                                        double dd = 0.0;
+                                        for (int x = 0; x < 3; x++) {
+                                            const double Tv = t0 * cell[0 * 3 + x] + t1 * cell[1 * 3 + x] + t2 * cell[2 * 3 + x];
+                                            t.A[x] = A[x];
+                                            t.Bt[x] = B[x] + Tv;
+                                            dd += (t.A[x] - t.Bt[x]) * (t.A[x] - t.Bt[x]);
+                                        }
+                                        if (!(std::sqrt(dd) < rsum)) continue;
+                                        const double aa = prim_exp[pa], ab = prim_exp[pb], ap = aa + ab;
+                                        double dA = 0.0, dB = 0.0;
+                                        for (int x = 0; x < 3; x++) {
+                                            t.P[x] = (aa * t.A[x] + ab * t.Bt[x]) / ap;
+                                            dA += (t.P[x] - t.A[x]) * (t.P[x] - t.A[x]);
+                                            dB += (t.P[x] - t.Bt[x]) * (t.P[x] - t.Bt[x]);
+                                        }
+                                        dA = std::sqrt(dA); dB = std::sqrt(dB);
+                                        const double ex = std::exp(-(aa * ab / ap) * dd);
+                                        const double kappa = std::fabs(prim_coef[pa] * prim_coef[pb]) * ex;
+                                        const double R = pair_radius(shl_l[sa], shl_l[sb], ap, kappa, dA, dB, tau);
+                                        if (R <= 0.0) continue;
+                                        int lev = 0;
+                                        for (int a = nlevel - 1; a >= 0; a--)
+                                            if (hp->lev[a].ecut >= rel_cutoff * ap) { lev = a; break; }
+                                        t.shl_a = (int)sa; t.prim_a = pa; t.shl_b = sb; t.prim_b = pb;
+                                        t.T[0] = t0; t.T[1] = t1; t.T[2] = t2;
+                                        t.level = lev; t.la = shl_l[sa]; t.lb = shl_l[sb];
+                                        t.R = R; t.ap = ap;
+                                        t.pref = prim_coef[pa] * prim_coef[pb] * ex;
+                                        t.sym = (hermi && !(pa == pb && t0 == 0 && t1 == 0 && t2 == 0)) ? 1 : 0;
+                                        outv.push_back(t);
+                                    }
+                        }
+            }
+        });
+        size_t nt = 0;
+        for (auto &v : per_shell) nt += v.size();
+        if (nt > 2000000000ull) { delete hp; set_error("gpw_build_pairs: more than 2^31 pairs"); return GPW_EUNSUPPORTED; }
+        hp->task.reserve(nt);
+        for (auto &v : per_shell) { hp->task.insert(hp->task.end(), v.begin(), v.end()); std::vector<HostTask>().swap(v); }
+        // sort by (level, L), keeping enumeration order inside a group
+        std::stable_sort(hp->task.begin(), hp->task.end(), [](const HostTask &x, const HostTask &y) {
+            if (x.level != y.level) return x.level < y.level;
+            return (x.la + x.lb) < (y.la + y.lb);
+        });
+        const long ntask = (long)hp->task.size();
+        hp->taskK.resize(ntask); hp->taskP.resize(ntask);
+        long long coff = 0;
+        for (long i = 0; i < ntask; i++) {
+            const HostTask &t = hp->task[i];
+            const LevelGeom &g = hp->lev[t.level];
+            TaskK &k = hp->taskK[i];
+            for (int a = 0; a < 3; a++)
+                k.nP[a] = (t.P[0] * hp->binv[0 * 3 + a] + t.P[1] * hp->binv[1 * 3 + a] + t.P[2] * hp->binv[2 * 3 + a]) * g.N[a];
+            k.ap = t.ap;
+            k.cc = std::exp(-2.0 * t.ap * g.Gm[2]);
+            k.coef_off = coff;
+            TaskP &p = hp->taskP[i];
+            for (int x = 0; x < 3; x++) { p.PA[x] = t.P[x] - t.A[x]; p.PB[x] = t.P[x] - t.Bt[x]; }
+            p.pref = t.pref; p.coef_off = coff;
+            p.ao_a = hp->ao_loc[t.shl_a]; p.ao_b = hp->ao_loc[t.shl_b];
+            p.la = (short)t.la; p.lb = (short)t.lb; p.level = (short)t.level; p.sym = (short)t.sym;
+            coff += ncoef_pad(t.la + t.lb);
+            hp->ntask_level[t.level]++;
+        }
+        hp->ncoef_total = coff;
+
+        // ---- T6: blocks of every pair ----
+        std::vector<long long> lev_tile0(nlevel + 1, 0);
+        for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;
+        const long long ntile_all = lev_tile0[nlevel];
+        // circumradius of a block about its centre (points at +-1.5 steps per axis)
+        std::vector<double> circ(nlevel);
+        for (int a = 0; a < nlevel; a++) {
+            double m = 0;
+            for (int sg = 0; sg < 4; sg++) {
+                double v[3];
+                for (int x = 0; x < 3; x++)
+                    v[x] = 1.5 * (hp->lev[a].H[x * 3 + 0] + ((sg & 1) ? -1 : 1) * hp->lev[a].H[x * 3 + 1] + ((sg & 2) ? -1 : 1) * hp->lev[a].H[x * 3 + 2]);
+                m = std::max(m, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+            }
+            circ[a] = m;
+        }
+        const long chunk = 256;
+        const long nchunk = (ntask + chunk - 1) / chunk;
+        std::vector<std::vector<RawVisit>> raw(nchunk);
+        std::atomic<int> wrap_overflow(0);
+        parallel_chunks(ntask, chunk, nthread, [&](long c, long lo, long hi, int) {
+            std::vector<RawVisit> &rv = raw[c];
+            for (long ti = lo; ti < hi; ti++) {
+                const HostTask &t = hp->task[ti];
+                const LevelGeom &g = hp->lev[t.level];
+                const int *N = g.N;
+                int blo[3], bhi[3];
+                for (int i = 0; i < 3; i++) {
+                    const double u = t.P[0] * hp->binv[0 * 3 + i] + t.P[1] * hp->binv[1 * 3 + i] + t.P[2] * hp->binv[2 * 3 + i];
+                    const double w = t.R * hp->bnorm[i] * N[i];
+                    blo[i] = floordiv((int)std::ceil(u * N[i] - w), TILE);
+                    bhi[i] = floordiv((int)std::floor(u * N[i] + w), TILE);
+                }
+                const double R2 = t.R * t.R;
+                const double rc = circ[t.level];
+                for (int b1 = blo[0]; b1 <= bhi[0]; b1++)
+                    for (int b2 = blo[1]; b2 <= bhi[1]; b2++)
+                        for (int b3 = blo[2]; b3 <= bhi[2]; b3++) {
+                            // quick decisions on the block centre; the 64-point test settles the rest
+                            double cpos[3], dc = 0;
+                            {
+                                const double u1 = (4 * b1 + 1.5) / N[0], u2 = (4 * b2 + 1.5) / N[1], u3 = (4 * b3 + 1.5) / N[2];
+                                for (int x = 0; x < 3; x++) {
+                                    cpos[x] = u1 * cell[0 * 3 + x] + u2 * cell[1 * 3 + x] + u3 * cell[2 * 3 + x];
+                                    dc += (cpos[x] - t.P[x]) * (cpos[x] - t.P[x]);
+                                }
+                                dc = std::sqrt(dc);
+                            }
+                            bool hit;
+                            if (dc - rc > t.R * (1.0 + 1e-9) + 1e-9) hit = false;
+                            else if (dc + rc < t.R * (1.0 - 1e-9) - 1e-9) hit = true;
+                            else {
+                                hit = false;
+                                for (int i = 0; i < 4 && !hit; i++)
+                                    for (int j = 0; j < 4 && !hit; j++)
+                                        for (int k = 0; k < 4 && !hit; k++) {
+                                            // r_n = (n1/N1) a1 + (n2/N2) a2 + (n3/N3) a3   (u0 = 0)
+                                            const double u1 = (double)(4 * b1 + i) / N[0], u2 = (double)(4 * b2 + j) / N[1],
+                                                         u3 = (double)(4 * b3 + k) / N[2];
+                                            double r[3];
+                                            for (int x = 0; x < 3; x++) r[x] = u1 * cell[0 * 3 + x] + u2 * cell[1 * 3 + x] + u3 * cell[2 * 3 + x];
+                                            const double d2 = (r[0] - t.P[0]) * (r[0] - t.P[0]) + (r[1] - t.P[1]) * (r[1] - t.P[1]) +
+                                                              (r[2] - t.P[2]) * (r[2] - t.P[2]);
+                                            if (d2 <= R2) hit = true;
+                                        }
+                            }
+                            if (!hit) continue;
+                            const int w1 = posmod(b1, g.T[0]), w2 = posmod(b2, g.T[1]), w3 = posmod(b3, g.T[2]);
+                            const int s1 = (b1 - w1) / g.T[0], s2 = (b2 - w2) / g.T[1], s3 = (b3 - w3) / g.T[2];
+                            if (s1 < -127 || s1 > 127 || s2 < -127 || s2 > 127 || s3 < -127 || s3 > 127) { wrap_overflow = 1; continue; }
+                            RawVisit v;
+                            v.key = lev_tile0[t.level] + ((long long)w1 * g.T[1] + w2) * g.T[2] + w3;
+                            v.task = (int)ti;
+                            v.s[0] = (signed char)s1; v.s[1] = (signed char)s2; v.s[2] = (signed char)s3;
+                            v.L = (unsigned char)(t.la + t.lb);
+                            rv.push_back(v);
+                        }
+            }
+        });
+        if (wrap_overflow) { delete hp; set_error("gpw_build_pairs: a pair wraps the cell more than 127 times"); return GPW_EUNSUPPORTED; }
+
+        // counting sort by block; chunks are in pair order, pairs are in (level, L) order, so every
+        // block's list comes out sorted by L
+        std::vector<long long> cnt(ntile_all + 1, 0);
+        std::vector<unsigned> segcnt((size_t)ntile_all * 8, 0);
+        long long nvis = 0;
+        for (auto &rv : raw) {
+            nvis += (long long)rv.size();
+            for (const RawVisit &v : rv) { cnt[v.key + 1]++; segcnt[(size_t)v.key * 8 + v.L]++; }
+        }
+        for (long long i = 0; i < ntile_all; i++) cnt[i + 1] += cnt[i];
+        hp->visit.resize((size_t)nvis);
+        {
+            std::vector<long long> cur(cnt.begin(), cnt.end() - 1);
+            for (auto &rv : raw) {
+                for (const RawVisit &v : rv) {
+                    Visit &o = hp->visit[(size_t)cur[v.key]++];
+                    o.task = v.task; o.s[0] = v.s[0]; o.s[1] = v.s[1]; o.s[2] = v.s[2]; o.pad = 0;
+                    const HostTask &t = hp->task[v.task];
+                    hp->nvisit_level[t.level]++;
+                    hp->nvisit_class[t.level][t.la][t.lb]++;
+                }
+                std::vector<RawVisit>().swap(rv);
+            }
+        }
+        hp->tile_base.resize(nlevel);
+        hp->seg.resize(nlevel);
+        for (int a = 0; a < nlevel; a++) {
+            const int ntl = hp->lev[a].ntile;
+            hp->tile_base[a].assign(cnt.begin() + lev_tile0[a], cnt.begin() + lev_tile0[a] + ntl + 1);
+            hp->seg[a].resize((size_t)ntl * 8);
+            for (int tl = 0; tl < ntl; tl++) {
+                unsigned acc = 0;
+                for (int L = 0; L < 8; L++) {
+                    hp->seg[a][(size_t)tl * 8 + L] = acc;
+                    acc += segcnt[(size_t)(lev_tile0[a] + tl) * 8 + L];
+                }
+            }
+        }
+        // ---- work items: every block's list cut into ranges of at most ITEM_MAX visits ----
+        const unsigned ITEM_MAX = 384;
+        for (int a = 0; a < nlevel; a++) {
+            const int ntl = hp->lev[a].ntile;
+            for (int tl = 0; tl < ntl; tl++) {
+                const unsigned n = (unsigned)(hp->tile_base[a][tl + 1] - hp->tile_base[a][tl]);
+                if (!n) continue;
+                const unsigned nparts = (n + ITEM_MAX - 1) / ITEM_MAX;
+                for (unsigned p = 0; p < nparts; p++) {
+                    Item it;
+                    it.level = a; it.tile = tl;
+                    it.lo = (unsigned)((unsigned long long)n * p / nparts);
+                    it.hi = (unsigned)((unsigned long long)n * (p + 1) / nparts);
+                    it.single = nparts == 1; it.pad = 0;
+                    hp->item.push_back(it);
+                }
+            }
+        }
+        std::stable_sort(hp->item.begin(), hp->item.end(),
+                         [](const Item &x, const Item &y) { return (x.hi - x.lo) > (y.hi - y.lo); });
+    } catch (const std::bad_alloc &) {
+        delete hp;
+        set_error("gpw_build_pairs: out of host memory");
+        return GPW_ENOMEM;
+    }
+    hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+    *out = hp;
+    return GPW_OK;
+}
+
+}  // namespace gpw

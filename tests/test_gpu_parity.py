@@ -1,0 +1,188 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element (-m gpu).
+
+Tolerance: 1e-11 relative to the max-norm, per level and component for rho, over all entries for F
+(north_star; T9).  Levels the oracle leaves exactly zero must be exactly zero."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2603_24881_b200 as gpw
+from paper_2603_24881_b200 import inputs
+
+from gpu_util import TOL, check_rho, gpu_mat, gpu_rho, relmax, tile_mask_to_points
+
+pytestmark = pytest.mark.gpu
+
+
+def _plan(inp, hermi=None):
+    a = list(inp.abi_args())
+    if hermi is not None:
+        a[14] = hermi
+    p = gpw.gpw_build_pairs(*a)
+    assert p.info["on_device"], "no device copy of the plan: the CUDA path did not run"
+    return p
+
+
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "wrap", "contracted", "resolved"])
+@pytest.mark.parametrize("deriv", [0, 1])
+@pytest.mark.parametrize("hermi", [1, 0])
+def test_small_cells_full_parity(kind, deriv, hermi):
+    inp = inputs.make_small(kind, deriv=deriv, hermi=hermi)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    if not hermi:   # ordered pairs must work for a non-symmetric D
+        D = D + 0.2 * np.random.default_rng(3).standard_normal(D.shape)
+    check_rho(gpu_rho(plan, D, deriv), o.eval_rho(D, deriv))
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    F, Fo = gpu_mat(plan, v, deriv), o.eval_mat(v, deriv)
+    assert np.isfinite(F).all()
+    assert relmax(F, Fo) <= TOL
+
+
+def test_hermi_uses_both_triangles_of_D():
+    """hermi = 1 processes unordered pairs with D_ab + D_ba: equals the ordered sum for any D."""
+    inp = inputs.make_small("contracted", deriv=1, hermi=1)
+    D = np.random.default_rng(5).standard_normal((inp.nao, inp.nao))
+    o = oracle.Oracle.from_inputs(inp)
+    check_rho(gpu_rho(_plan(inp), D, 1), o.eval_rho(D, 1))
+
+
+def test_config0_full():
+    inp = inputs.make_config(0)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    for deriv in (0, 1):
+        check_rho(gpu_rho(plan, D, deriv), o.eval_rho(D, deriv))
+        v = [inp.v(l, 4 if deriv else 1) for l in range(inp.nlevel)]
+        assert relmax(gpu_mat(plan, v, deriv), o.eval_mat(v, deriv)) <= TOL
+
+
+def test_config1_full_32_water():
+    inp = inputs.make_config(1)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    rho = gpu_rho(plan, D, 0)
+    check_rho(rho, o.eval_rho(D, 0))
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    F = gpu_mat(plan, v, 0)
+    assert relmax(F, o.eval_mat(v, 0)) <= TOL
+    # adjointness on the GPU outputs alone (pin G6)
+    vol = abs(np.linalg.det(inp.cell))
+    lhs = sum(np.sum(r * x) * vol / r[0].size for r, x in zip(rho, v))
+    assert abs(lhs - np.sum(D * F)) <= 1e-11 * max(abs(lhs), 1.0)
+
+
+def _sampled_parity(inp, tile_frac, pair_frac, seed=0):
+    """Full-size launch, oracle on a seeded sample: all visits of the sampled blocks (rho) and all
+    visits of the sampled shell pairs (F)."""
+    rng = np.random.default_rng(seed)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    masks = []
+    for lev in range(inp.nlevel):
+        nt = int(np.prod(inp.mesh[lev] // 4))
+        m = rng.random(nt) < max(tile_frac, min(1.0, 8.0 / nt))
+        masks.append(m.astype(np.uint8))
+    got = gpu_rho(plan, D, inp.deriv)
+    want = o.eval_rho(D, inp.deriv, tile_masks=masks)
+    for lev in range(inp.nlevel):
+        pm = tile_mask_to_points(masks[lev], inp.mesh[lev])
+        for c in range(want[lev].shape[0]):
+            assert np.isfinite(got[lev][c]).all()
+            ref = np.abs(got[lev][c]).max()
+            if ref == 0.0:
+                assert not np.any(want[lev][c])
+                continue
+            e = np.abs(got[lev][c][pm] - want[lev][c][pm]).max() / ref
+            assert e <= TOL, f"rho level {lev} comp {c}: rel err {e:.3e}"
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    F = gpu_mat(plan, v, inp.deriv)
+    assert np.isfinite(F).all()
+    pmask = (rng.random((inp.nshl, inp.nshl)) < pair_frac).astype(np.uint8)
+    Fo = o.eval_mat(v, inp.deriv, pair_mask=pmask)
+    loc = inp.ao_loc
+    sel = np.zeros((inp.nao, inp.nao), bool)
+    for sa, sb in zip(*np.nonzero(pmask)):
+        sel[loc[sa]:loc[sa + 1], loc[sb]:loc[sb + 1]] = True
+    e = np.abs(F[sel] - Fo[sel]).max() / np.abs(F).max()
+    assert e <= TOL, f"F rel err {e:.3e}"
+    assert np.abs(F - F.T).max() <= 1e-12 * np.abs(F).max()
+    # adjointness on the full GPU outputs (pin G6): exact for any truncation
+    vol = abs(np.linalg.det(inp.cell))
+    lhs = sum(np.sum(r * x) * vol / r[0].size for r, x in zip(got, v))
+    assert abs(lhs - np.sum(D * F)) <= 1e-11 * max(abs(lhs), 1.0)
+
+
+def test_config3_f_shells_triclinic_sampled():
+    _sampled_parity(inputs.make_config(3), tile_frac=0.004, pair_frac=0.0015)
+
+
+def test_config2_256_water_gga_sampled():
+    _sampled_parity(inputs.make_config(2), tile_frac=0.0008, pair_frac=0.00004)
+
+
+# ------------------------------------------------------------------------------------------ edge cases
+def test_empty_plan_and_empty_levels():
+    base = inputs.make_small("cubic", deriv=1)
+    # (i) threshold so loose that every primitive is dropped: outputs are exactly zero
+    inp = dataclasses.replace(base, tau=1e6)
+    plan = _plan(inp)
+    assert plan.info["ntask"] == 0
+    rho = gpu_rho(plan, inp.D(), 1)
+    assert all(not np.any(r) for r in rho)
+    assert not np.any(gpu_mat(plan, [inp.v(l) for l in range(inp.nlevel)], 1))
+    # (ii) a coarse level no pair is assigned to stays exactly zero
+    inp = dataclasses.replace(base, mesh=np.array([[28, 28, 28], [8, 8, 8]], np.int32))
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    assert plan.info["ntask_level"][1] == 0
+    rho = gpu_rho(plan, inp.D(), 1)
+    assert not np.any(rho[1])
+    check_rho(rho, o.eval_rho(inp.D(), 1))
+
+
+def test_single_s_primitive_and_minimal_mesh():
+    """One s function on the smallest legal mesh (one 4x4x4 block per axis pair, many wraps)."""
+    cell = np.eye(3) * 3.0
+    inp = inputs.make_custom(cell, [[0.4, 1.1, 2.0]], [[(0, [0.9], [1.3])]], [[4, 8, 4]], C=np.ones((1, 1)),
+                             tau=1e-10, deriv=1)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = np.ones((1, 1))
+    check_rho(gpu_rho(plan, D, 1), o.eval_rho(D, 1))
+    v = [inp.v(0)]
+    assert relmax(gpu_mat(plan, v, 1), o.eval_mat(v, 1)) <= TOL
+
+
+def test_long_visit_lists_split_into_items():
+    """Diffuse f shells on a coarse mesh: every block is visited by every pair many times over, so the
+    lists are cut into several work items that accumulate atomically."""
+    cell = np.array([[6.0, 0.3, 0.0], [0.0, 6.2, 0.4], [0.5, 0.0, 5.8]])
+    rng = np.random.default_rng(9)
+    xyz = rng.uniform(0, 6, (6, 3))
+    shells = [[(0, [0.21], [1.0]), (1, [0.17], [0.8]), (2, [0.25], [0.6]), (3, [0.19], [0.5])] for _ in range(6)]
+    inp = inputs.make_custom(cell, xyz, shells, [[12, 12, 12]], tau=1e-10, deriv=1, seed=2)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    assert plan.info["nitem"] > 27          # more items than blocks
+    D = inp.D()
+    check_rho(gpu_rho(plan, D, 1), o.eval_rho(D, 1))
+    v = [inp.v(0)]
+    assert relmax(gpu_mat(plan, v, 1), o.eval_mat(v, 1)) <= TOL
+
+
+def test_repeat_calls_overwrite_outputs():
+    inp = inputs.make_small("cubic", deriv=0)
+    plan = _plan(inp)
+    D = inp.D()
+    r1 = gpu_rho(plan, D, 0)
+    r2 = gpu_rho(plan, 2.0 * D, 0)
+    assert relmax(r2[0], 2.0 * r1[0]) <= 1e-13
+    v = [inp.v(0)]
+    assert relmax(gpu_mat(plan, v, 0), gpu_mat(plan, v, 0)) <= 1e-13
