@@ -150,6 +150,16 @@ int gpw_plan_info(const gpw_plan *plan, gpw_info *out);
 int gpw_plan_export_tasks(const gpw_plan *plan, gpw_task *host_buf, long cap, long *ntask);
 
 /*
+ * Measurement aid: with timing enabled the eval calls bracket each of their kernels with CUDA events on
+ * the call's stream (no synchronisation is added).  gpw_plan_get_timing waits for the last call of the
+ * given kind (which = 0: gpw_eval_rho, 1: gpw_eval_mat) and writes two durations in milliseconds to the
+ * HOST array ms_out[2]:  which = 0: {pre-pass D -> pair polynomials, collocation kernel};
+ * which = 1: {integration kernel, post-pass pair moments -> F}.
+ */
+int gpw_plan_set_timing(gpw_plan *plan, int enable);
+int gpw_plan_get_timing(gpw_plan *plan, int which, float *ms_out);
+
+/*
  * Measurement aid: FP64 FMA throughput of the current device (register-only DFMA loop on every SM, 8
  * independent chains per thread, best launch over at least min_seconds), in TFLOP/s.  The denominator
  * of the "alu" roofline that bench.py reports.  Host pointers; synchronises the device.

@@ -64,6 +64,7 @@ def _load():
     L.orc_nao.argtypes = [ctypes.c_void_p]
     L.orc_get_tasks.argtypes = [ctypes.c_void_p, _ip, _dp]
     L.orc_visit_counts.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_long)]
+    L.orc_last_visit_counts.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_long)]
     L.orc_eval_rho.restype = ctypes.c_int
     L.orc_eval_rho.argtypes = [ctypes.c_void_p, _dp, ctypes.c_int, ctypes.POINTER(_dp),
                                ctypes.POINTER(_ucp)]
@@ -151,6 +152,12 @@ class Oracle:
         """[nlevel,4,4] number of (ordered task, 4x4x4 tile) visits per (la, lb)."""
         out = np.zeros((self.nlevel, 4, 4), dtype=np.int64)
         self._L.orc_visit_counts(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_long)))
+        return out
+
+    def last_visit_counts(self) -> np.ndarray:
+        """[nlevel,4,4] visits evaluated by the last eval_rho / eval_mat call (bookkeeping for timing)."""
+        out = np.zeros((self.nlevel, 4, 4), dtype=np.int64)
+        self._L.orc_last_visit_counts(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_long)))
         return out
 
     def eval_rho(self, D: np.ndarray, deriv: int = 0,

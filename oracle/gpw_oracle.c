@@ -69,6 +69,7 @@ typedef struct {
     long ntask;
     orc_task *task;
     int visits_built; /* 0 = none, 1 = all */
+    long last_counts[8 * 16]; /* (ordered pair, tile) visits evaluated by the last eval call, [level][la][lb] */
 } orc_ctx;
 
 static int ncart(int l) { return (l + 1) * (l + 2) / 2; }
@@ -391,6 +392,15 @@ static void build_visits(orc_ctx *c, const unsigned char *const *tile_mask, cons
         task_tiles(c, k, m, 1);
     }
     c->visits_built = 1;
+    memset(c->last_counts, 0, sizeof(c->last_counts));
+    for (long t = 0; t < c->ntask; t++)
+        c->last_counts[c->task[t].level * 16 + c->task[t].la * 4 + c->task[t].lb] += c->task[t].nvis;
+}
+
+/* bookkeeping only (used to size the timed CPU baseline): visits the last eval call evaluated */
+void orc_last_visit_counts(const orc_ctx *c, long *counts)
+{
+    memcpy(counts, c->last_counts, sizeof(long) * c->nlevel * 16);
 }
 
 /* T7/T8 collocation.  D: [nao][nao] row-major.  rho[level]: [ncomp][N1][N2][N3],

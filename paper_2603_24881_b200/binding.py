@@ -51,7 +51,8 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _lib = None
 
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_interp_up", "gpw_restrict_down",
-           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak"]
+           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
+           "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
 
 def load_library():
@@ -83,6 +84,10 @@ def load_library():
     L.gpw_plan_export_tasks.restype = ctypes.c_int
     L.gpw_plan_export_tasks.argtypes = [ctypes.c_void_p, ctypes.POINTER(gpw_task), ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_long)]
+    L.gpw_plan_set_timing.restype = ctypes.c_int
+    L.gpw_plan_set_timing.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    L.gpw_plan_get_timing.restype = ctypes.c_int
+    L.gpw_plan_get_timing.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
     L.gpw_dfma_peak.restype = ctypes.c_int
     L.gpw_dfma_peak.argtypes = [ctypes.c_double, _dp, _ip]
     L.gpw_free_plan.restype = None
@@ -206,6 +211,18 @@ def gpw_interp_up(plan: Plan, rho: Sequence, ncomp: int, rho_fine, stream=None):
 def gpw_restrict_down(plan: Plan, v_fine, ncomp: int, v: Sequence, stream=None):
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
     _check(load_library().gpw_restrict_down(plan._h, ctypes.c_void_p(v_fine.data_ptr()), int(ncomp), ptrs, _stream_ptr(stream)))
+
+
+def gpw_plan_set_timing(plan: Plan, enable: bool):
+    _check(load_library().gpw_plan_set_timing(plan._h, int(bool(enable))))
+
+
+def gpw_plan_get_timing(plan: Plan, which: int):
+    """Kernel durations (ms) of the last eval_rho (which=0: pre-pass, collocation) or eval_mat
+    (which=1: integration, post-pass); waits for that call to finish."""
+    ms = (ctypes.c_float * 2)()
+    _check(load_library().gpw_plan_get_timing(plan._h, int(which), ms))
+    return float(ms[0]), float(ms[1])
 
 
 def gpw_dfma_peak(min_seconds: float = 0.5):

@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpw.so")
-SOURCES = ["plan.cpp", "gpw_cuda.cu"]
-HEADERS = ["gpw_internal.h", "gpw_math.cuh"]
+SOURCES = ["plan.cpp", "gpw_api.cu", "collocate.cu", "integrate.cu"]
+HEADERS = ["gpw_internal.h", "gpw_math.cuh", "gpw_kernels.cuh"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O3", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

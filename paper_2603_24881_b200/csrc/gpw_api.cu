@@ -1,13 +1,9 @@
-// CUDA kernels (sm_100a) and the C ABI of include/gpw.h.
+// The C ABI of include/gpw.h, the pre/post-pass kernels and the FP64 peak probe (sm_100a).
 //
 // Kernels:
 //   k_poly_from_D       pre-pass: one thread per pair, D block -> polynomial about P in grid-index coordinates
-//   k_collocate<DERIV>  Eq. (3): one warp per work item (a 4x4x4 block and a range of its visit list);
-//                       a half-warp evaluates one (pair, block) visit, a lane owns a column of 4 points
-//                       and keeps its rho values in registers; one store (or atomic add) per point at the end
-//   k_integrate<DERIV>  Eq. (4): same decomposition; the block of v lives in registers, each visit's
-//                       moment vector is reduced over the half-warp by a shuffle reduce-scatter and added
-//                       to the pair's moment vector
+//   k_collocate         collocate.cu
+//   k_integrate         integrate.cu
 //   k_F_from_moments    post-pass: one thread per pair, moments -> F block (x dV), atomics into F
 #include <cuda_runtime.h>
 
@@ -16,17 +12,10 @@
 #include <cstring>
 #include <new>
 
-#include "gpw_math.cuh"
+#include "gpw_kernels.cuh"
 
 namespace gpw {
 const char *last_error_cstr();
-
-struct GridParams {
-    LevelGeom lev[GPW_MAX_LEVEL];
-    const long long *tile_base[GPW_MAX_LEVEL];
-    const unsigned *seg[GPW_MAX_LEVEL];
-    double *grid[GPW_MAX_LEVEL];   // rho (written) or v (read)
-};
 
 // ------------------------------------------------------------------------------------------ pre/post pass
 __global__ void __launch_bounds__(128) k_poly_from_D(const TaskP *__restrict__ tp, int ntask,
@@ -56,235 +45,6 @@ __global__ void __launch_bounds__(128) k_F_from_moments(const TaskP *__restrict_
             atomicAdd(F + (size_t)(p.ao_a + i) * nao + p.ao_b + j, x);
             if (p.sym) atomicAdd(F + (size_t)(p.ao_b + j) * nao + p.ao_a + i, x);
         }
-}
-
-// ------------------------------------------------------------------------------------------ collocation
-struct VisitCtx {
-    const TaskK *tasks;
-    const Visit *visits;   // already offset to the block's list
-    const double *work;    // polynomial workspace
-    double gm[6];
-    int n1, n2, n3;        // stored index of the lane's column start
-    int N0, N1, N2;
-};
-
-struct LoadedVisit {
-    double u1, u2, u30, ap, cc;
-    long long coef_off;
-};
-
-__device__ __forceinline__ LoadedVisit load_visit(const VisitCtx &c, unsigned v) {
-    const Visit vi = c.visits[v];
-    const double2 *tk = reinterpret_cast<const double2 *>(c.tasks + vi.task);
-    const double2 a = __ldg(tk), b = __ldg(tk + 1), d = __ldg(tk + 2);
-    LoadedVisit r;
-    r.u1 = (double)(c.n1 + vi.s[0] * c.N0) - a.x;
-    r.u2 = (double)(c.n2 + vi.s[1] * c.N1) - a.y;
-    r.u30 = (double)(c.n3 + vi.s[2] * c.N2) - b.x;
-    r.ap = b.y;
-    r.cc = d.x;
-    r.coef_off = __double_as_longlong(d.y);
-    return r;
-}
-
-template <int L, int DERIV>
-__device__ __forceinline__ void colloc_segment(const VisitCtx &c, unsigned lo, unsigned hi, int half,
-                                               double (*acc)[4]) {
-    for (unsigned v = lo + half; v < hi; v += 2) {
-        const LoadedVisit lv = load_visit(c, v);
-        double q[6];
-#pragma unroll
-        for (int x = 0; x < 6; x++) q[x] = lv.ap * c.gm[x];
-        colloc_column<L, DERIV>(c.work + lv.coef_off, q, lv.cc, lv.u1, lv.u2, lv.u30, acc);
-    }
-}
-
-template <int DERIV>
-__global__ void __launch_bounds__(128) k_collocate(const __grid_constant__ GridParams P,
-                                                    const TaskK *__restrict__ tasks,
-                                                    const Visit *__restrict__ visits,
-                                                    const Item *__restrict__ items, int nitem,
-                                                    const double *__restrict__ coef) {
-    constexpr int NCOMP = DERIV ? 4 : 1;
-    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (w >= nitem) return;
-    const Item it = items[w];
-    const LevelGeom &g = P.lev[it.level];
-    const int lane = threadIdx.x & 31, half = lane >> 4, col = lane & 15;
-    const int T2 = g.T[2], T1 = g.T[1];
-    const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
-    VisitCtx c;
-    c.tasks = tasks;
-    c.visits = visits + P.tile_base[it.level][it.tile];
-    c.work = coef;
-#pragma unroll
-    for (int x = 0; x < 6; x++) c.gm[x] = g.Gm[x];
-    c.n1 = 4 * b1 + (col >> 2); c.n2 = 4 * b2 + (col & 3); c.n3 = 4 * b3;
-    c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
-    const unsigned *seg = P.seg[it.level] + (size_t)it.tile * 8;
-
-    double acc[NCOMP][4];
-#pragma unroll
-    for (int k = 0; k < NCOMP; k++)
-#pragma unroll
-        for (int t = 0; t < 4; t++) acc[k][t] = 0.0;
-
-#pragma unroll 1
-    for (int L = 0; L <= MAXLP; L++) {
-        const unsigned lo = max(it.lo, seg[L]), hi = min(it.hi, seg[L + 1]);
-        if (lo >= hi) continue;
-        switch (L) {
-            case 0: colloc_segment<0, DERIV>(c, lo, hi, half, acc); break;
-            case 1: colloc_segment<1, DERIV>(c, lo, hi, half, acc); break;
-            case 2: colloc_segment<2, DERIV>(c, lo, hi, half, acc); break;
-            case 3: colloc_segment<3, DERIV>(c, lo, hi, half, acc); break;
-            case 4: colloc_segment<4, DERIV>(c, lo, hi, half, acc); break;
-            case 5: colloc_segment<5, DERIV>(c, lo, hi, half, acc); break;
-            default: colloc_segment<6, DERIV>(c, lo, hi, half, acc); break;
-        }
-    }
-    // the two half-warps worked on alternate visits of the same block
-#pragma unroll
-    for (int k = 0; k < NCOMP; k++)
-#pragma unroll
-        for (int t = 0; t < 4; t++) acc[k][t] += __shfl_xor_sync(0xffffffffu, acc[k][t], 16);
-    if (half) return;
-    const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
-    double *out = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2) * g.N[2] + c.n3;
-    double res[NCOMP][4];
-#pragma unroll
-    for (int t = 0; t < 4; t++) {
-        res[0][t] = acc[0][t];
-        if constexpr (DERIV) {
-            // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-                res[1 + x][t] = g.Hinv[0 * 3 + x] * acc[1][t] + g.Hinv[1 * 3 + x] * acc[2][t] +
-                                g.Hinv[2 * 3 + x] * acc[3][t];
-        }
-    }
-    if (it.single) {
-#pragma unroll
-        for (int k = 0; k < NCOMP; k++) {
-            double2 *o = reinterpret_cast<double2 *>(out + k * ng);
-            o[0] = make_double2(res[k][0], res[k][1]);
-            o[1] = make_double2(res[k][2], res[k][3]);
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < NCOMP; k++)
-#pragma unroll
-            for (int t = 0; t < 4; t++) atomicAdd(out + k * ng + t, res[k][t]);
-    }
-}
-
-// ------------------------------------------------------------------------------------------ integration
-// Sum an N-vector held by each of the 16 lanes of a half-warp; afterwards lane j holds elements
-// [j*N/16, (j+1)*N/16) of the total in m[0 .. N/16).  N is a multiple of 16.
-template <int N>
-__device__ __forceinline__ void halfwarp_reduce_scatter(double *m, int lane) {
-    static_assert(N % 16 == 0, "pad to a multiple of 16");
-#pragma unroll
-    for (int step = 0; step < 4; step++) {
-        const int bit = 8 >> step;
-        const int len = N >> (step + 1);
-        const bool up = lane & bit;
-#pragma unroll
-        for (int i = 0; i < len; i++) {
-            const double send = up ? m[i] : m[i + len];
-            const double keep = up ? m[i + len] : m[i];
-            m[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
-        }
-    }
-}
-
-template <int L, int DERIV>
-__device__ __forceinline__ void integ_segment(const VisitCtx &c, unsigned lo, unsigned hi, int lane,
-                                              const double (*vv)[4], double *__restrict__ mom) {
-    constexpr int NC = ncoef(L);
-    constexpr int NPAD = (NC + 15) / 16 * 16;
-    constexpr int PER = NPAD / 16;
-    const int half = lane >> 4;
-    for (unsigned v0 = lo; v0 < hi; v0 += 2) {   // warp-uniform trip count: the shuffles need every lane
-        const unsigned v = v0 + half;
-        const bool active = v < hi;
-        const LoadedVisit lv = load_visit(c, active ? v : lo);
-        double q[6];
-#pragma unroll
-        for (int x = 0; x < 6; x++) q[x] = lv.ap * c.gm[x];
-        double m[NPAD];
-#pragma unroll
-        for (int i = 0; i < NPAD; i++) m[i] = 0.0;
-        integ_column<L, DERIV>(vv, q, lv.cc, lv.u1, lv.u2, lv.u30, m);
-        halfwarp_reduce_scatter<NPAD>(m, lane);
-        if (active) {
-            double *dst = mom + lv.coef_off + (lane & 15) * PER;
-#pragma unroll
-            for (int i = 0; i < PER; i++)
-                if ((lane & 15) * PER + i < NC) atomicAdd(dst + i, m[i]);
-        }
-    }
-}
-
-template <int DERIV>
-__global__ void __launch_bounds__(128) k_integrate(const __grid_constant__ GridParams P,
-                                                    const TaskK *__restrict__ tasks,
-                                                    const Visit *__restrict__ visits,
-                                                    const Item *__restrict__ items, int nitem,
-                                                    double *__restrict__ mom) {
-    constexpr int NCOMP = DERIV ? 4 : 1;
-    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (w >= nitem) return;
-    const Item it = items[w];
-    const LevelGeom &g = P.lev[it.level];
-    const int lane = threadIdx.x & 31, col = lane & 15;
-    const int T2 = g.T[2], T1 = g.T[1];
-    const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
-    VisitCtx c;
-    c.tasks = tasks;
-    c.visits = visits + P.tile_base[it.level][it.tile];
-    c.work = nullptr;
-#pragma unroll
-    for (int x = 0; x < 6; x++) c.gm[x] = g.Gm[x];
-    c.n1 = 4 * b1 + (col >> 2); c.n2 = 4 * b2 + (col & 3); c.n3 = 4 * b3;
-    c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
-    const unsigned *seg = P.seg[it.level] + (size_t)it.tile * 8;
-
-    // the lane's column of v; for DERIV the vector field is mapped to grid-index components,
-    // w'_i = sum_c Hinv[i][c] w_c, so that w . grad_r f = w' . grad_u f
-    const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
-    const double *in = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2) * g.N[2] + c.n3;
-    double raw[NCOMP][4], vv[NCOMP][4];
-#pragma unroll
-    for (int k = 0; k < NCOMP; k++) {
-        const double2 *p2 = reinterpret_cast<const double2 *>(in + k * ng);
-        const double2 x0 = __ldg(p2), x1 = __ldg(p2 + 1);
-        raw[k][0] = x0.x; raw[k][1] = x0.y; raw[k][2] = x1.x; raw[k][3] = x1.y;
-    }
-#pragma unroll
-    for (int t = 0; t < 4; t++) {
-        vv[0][t] = raw[0][t];
-        if constexpr (DERIV) {
-#pragma unroll
-            for (int i = 0; i < 3; i++)
-                vv[1 + i][t] = g.Hinv[i * 3 + 0] * raw[1][t] + g.Hinv[i * 3 + 1] * raw[2][t] +
-                               g.Hinv[i * 3 + 2] * raw[3][t];
-        }
-    }
-#pragma unroll 1
-    for (int L = 0; L <= MAXLP; L++) {
-        const unsigned lo = max(it.lo, seg[L]), hi = min(it.hi, seg[L + 1]);
-        if (lo >= hi) continue;
-        switch (L) {
-            case 0: integ_segment<0, DERIV>(c, lo, hi, lane, vv, mom); break;
-            case 1: integ_segment<1, DERIV>(c, lo, hi, lane, vv, mom); break;
-            case 2: integ_segment<2, DERIV>(c, lo, hi, lane, vv, mom); break;
-            case 3: integ_segment<3, DERIV>(c, lo, hi, lane, vv, mom); break;
-            case 4: integ_segment<4, DERIV>(c, lo, hi, lane, vv, mom); break;
-            case 5: integ_segment<5, DERIV>(c, lo, hi, lane, vv, mom); break;
-            default: integ_segment<6, DERIV>(c, lo, hi, lane, vv, mom); break;
-        }
-    }
 }
 
 // ------------------------------------------------------------------------------------------ FP64 peak probe
@@ -319,11 +79,18 @@ struct gpw_plan {
     TaskP *d_taskP = nullptr;
     Visit *d_visit = nullptr;
     Item *d_item = nullptr;
+    BEntry *d_bentry = nullptr;
+    BItem *d_bitem = nullptr;
+    long long *d_brick_base[GPW_MAX_LEVEL] = {nullptr};
     double *d_S = nullptr;
     long long *d_tile_base[GPW_MAX_LEVEL] = {nullptr};
     unsigned *d_seg[GPW_MAX_LEVEL] = {nullptr};
     double *d_coef = nullptr;   // polynomial workspace of gpw_eval_rho
     double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
+    // optional kernel timing (gpw_plan_set_timing): events around each kernel of the last eval calls
+    bool timing = false;
+    cudaEvent_t ev[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    bool ev_valid[2] = {false, false};
 };
 
 namespace {
@@ -345,8 +112,12 @@ bool upload(T **dst, const T *src, size_t n, long &bytes, const char *what) {
 }
 
 void free_device(gpw_plan *p) {
+    for (int w = 0; w < 2; w++)
+        for (int k = 0; k < 3; k++)
+            if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
     cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_visit); cudaFree(p->d_item); cudaFree(p->d_S);
-    cudaFree(p->d_coef); cudaFree(p->d_mom);
+    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_bentry); cudaFree(p->d_bitem);
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) cudaFree(p->d_brick_base[a]);
     for (int a = 0; a < GPW_MAX_LEVEL; a++) { cudaFree(p->d_tile_base[a]); cudaFree(p->d_seg[a]); }
 }
 
@@ -357,6 +128,7 @@ void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
         P.lev[a] = hp->lev[a];
         P.tile_base[a] = p->d_tile_base[a];
         P.seg[a] = p->d_seg[a];
+        P.brick_base[a] = p->d_brick_base[a];
         P.grid[a] = grids[a];
     }
 }
@@ -393,6 +165,8 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     ok = ok && upload(&p->d_taskP, hp->taskP.data(), hp->taskP.size(), nb, "upload pairs");
     ok = ok && upload(&p->d_visit, hp->visit.data(), hp->visit.size(), nb, "upload visit lists");
     ok = ok && upload(&p->d_item, hp->item.data(), hp->item.size(), nb, "upload work items");
+    ok = ok && upload(&p->d_bentry, hp->bentry.data(), hp->bentry.size(), nb, "upload brick lists");
+    ok = ok && upload(&p->d_bitem, hp->bitem.data(), hp->bitem.size(), nb, "upload brick work items");
     if (ok) {
         std::vector<double> S_all((size_t)hp->nlevel * S_TOTAL);
         for (int a = 0; a < hp->nlevel; a++) std::memcpy(S_all.data() + (size_t)a * S_TOTAL, hp->S[a].data(), sizeof(double) * S_TOTAL);
@@ -401,6 +175,7 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     for (int a = 0; a < hp->nlevel && ok; a++) {
         ok = ok && upload(&p->d_tile_base[a], hp->tile_base[a].data(), hp->tile_base[a].size(), nb, "upload block offsets");
         ok = ok && upload(&p->d_seg[a], hp->seg[a].data(), hp->seg[a].size(), nb, "upload block segments");
+        ok = ok && upload(&p->d_brick_base[a], hp->brick_base[a].data(), hp->brick_base[a].size(), nb, "upload brick offsets");
     }
     const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
     ok = ok && cuda_ok(cudaMalloc((void **)&p->d_coef, sizeof(double) * nw), "allocate polynomial workspace");
@@ -476,12 +251,15 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     }
     const int ntask = (int)hp->task.size(), nitem = (int)hp->item.size();
     if (ntask == 0 || nitem == 0) return GPW_OK;
+    gpw_plan *pm = const_cast<gpw_plan *>(p);
+    if (p->timing) { cudaEventRecord(p->ev[0][0], st); pm->ev_valid[0] = true; }
     k_poly_from_D<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, D_dev, hp->nao, p->d_S, p->d_coef);
+    if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    const int nblk = (nitem + 3) / 4;
-    if (deriv) k_collocate<1><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef);
-    else k_collocate<0><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef);
+    if (!cuda_ok(launch_collocate(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, st),
+                 "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
+    if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
     return GPW_OK;
 }
@@ -500,13 +278,37 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     if (!cuda_ok(cudaMemsetAsync(p->d_mom, 0, sizeof(double) * (size_t)hp->ncoef_total, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     GridParams P;
     fill_params(p, P, const_cast<double *const *>(v_dev));
-    const int nblk = (nitem + 3) / 4;
-    if (deriv) k_integrate<1><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_mom);
-    else k_integrate<0><<<nblk, 128, 0, st>>>(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_mom);
+    gpw_plan *pm = const_cast<gpw_plan *>(p);
+    if (p->timing) { cudaEventRecord(p->ev[1][0], st); pm->ev_valid[1] = true; }
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->d_bentry, p->d_bitem, (int)hp->bitem.size(), p->d_mom, deriv,
+                                  hp->max_L, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
+    if (p->timing) cudaEventRecord(p->ev[1][1], st);
     DVs dv;
     for (int a = 0; a < GPW_MAX_LEVEL; a++) dv.v[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;
     k_F_from_moments<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, p->d_mom, p->d_S, dv, F_dev, hp->nao);
+    if (p->timing) cudaEventRecord(p->ev[1][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat: kernel launch")) return GPW_ECUDA;
+    return GPW_OK;
+}
+
+int gpw_plan_set_timing(gpw_plan *p, int enable) {
+    if (!p) { set_error("gpw_plan_set_timing: null plan"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_plan_set_timing: the plan has no device copy"); return GPW_ECUDA; }
+    if (enable && !p->ev[0][0])
+        for (int w = 0; w < 2; w++)
+            for (int k = 0; k < 3; k++)
+                if (!cuda_ok(cudaEventCreate(&p->ev[w][k]), "gpw_plan_set_timing")) return GPW_ECUDA;
+    p->timing = enable != 0;
+    p->ev_valid[0] = p->ev_valid[1] = false;
+    return GPW_OK;
+}
+
+int gpw_plan_get_timing(gpw_plan *p, int which, float *ms_out) {
+    if (!p || !ms_out || which < 0 || which > 1) { set_error("gpw_plan_get_timing: bad argument"); return GPW_EINVAL; }
+    if (!p->timing || !p->ev_valid[which]) { set_error("gpw_plan_get_timing: no timed call of that kind yet"); return GPW_EINVAL; }
+    if (!cuda_ok(cudaEventSynchronize(p->ev[which][2]), "gpw_plan_get_timing")) return GPW_ECUDA;
+    cudaEventElapsedTime(&ms_out[0], p->ev[which][0], p->ev[which][1]);
+    cudaEventElapsedTime(&ms_out[1], p->ev[which][1], p->ev[which][2]);
     return GPW_OK;
 }
 

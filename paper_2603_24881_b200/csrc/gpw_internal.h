@@ -19,6 +19,8 @@ constexpr int MAXL = GPW_MAX_L;          // shells up to f
 constexpr int MAXLP = 2 * MAXL;          // pair polynomial degree L = la + lb <= 6
 constexpr int NLSEG = MAXLP + 1;         // visit lists are segmented by L = 0..6
 constexpr int TILE = 4;                  // grid block edge
+constexpr int BRICK = 3;                 // integration stages bricks of BRICK^3 grid blocks in shared memory
+constexpr int BRICK_TILES = BRICK * BRICK * BRICK;
 
 // number of monomials u1^kx u2^ky u3^kz with kx+ky+kz <= L
 GPW_CX int ncoef(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
@@ -31,6 +33,8 @@ struct LevelGeom {
     int N[3];        // mesh
     int T[3];        // 4x4x4 blocks per axis
     int ntile;       // T[0]*T[1]*T[2]
+    int nbrick;      // B[0]*B[1]*B[2]
+    int B[3];        // bricks per axis, ceil(T / BRICK) (the last brick of an axis may be ragged)
     int pad0;
     double H[9];     // H[c*3+i] = component c of the grid step vector a_i / N_i :  r - P = H (n - n_P)
     double Hinv[9];  // Hinv[i*3+c]:  u_i = sum_c Hinv[i*3+c] X_c
@@ -77,6 +81,23 @@ struct Item {
     int pad;
 };
 
+// One (pair, lattice image, brick) entry of a brick's list: which of the brick's blocks the pair visits.
+struct BEntry {
+    int task;
+    signed char s[3];     // lattice wraps of this image
+    unsigned char L;      // la + lb
+    unsigned mask;        // bit ((t1*BRICK + t2)*BRICK + t3) set: block (t1,t2,t3) of the brick is visited
+    unsigned pad;
+};
+static_assert(sizeof(BEntry) == 16, "BEntry must be 16 bytes");
+
+// Work item of the integration kernel: a range of one brick's entry list.
+struct BItem {
+    int level;
+    int brick;
+    unsigned lo, hi;      // entry range relative to the brick's list
+};
+
 struct HostTask {
     int shl_a, prim_a, shl_b, prim_b;
     int T[3];
@@ -103,6 +124,10 @@ struct HostPlan {
     std::vector<std::vector<unsigned>> seg;          // [level][ntile*8] start of each L segment (relative)
     std::vector<Visit> visit;                        // all levels, level-major, block-major
     std::vector<Item> item;                          // sorted by descending size
+    std::vector<std::vector<long long>> brick_base;  // [level][nbrick+1] global entry index
+    std::vector<BEntry> bentry;                      // all levels, level-major, brick-major, sorted by L
+    std::vector<BItem> bitem;                        // sorted by descending work
+    int max_L = 0;                                   // largest la + lb present
     long nvisit_level[GPW_MAX_LEVEL] = {0};
     long ntask_level[GPW_MAX_LEVEL] = {0};
     long nvisit_class[GPW_MAX_LEVEL][MAXL + 1][MAXL + 1] = {{{0}}};

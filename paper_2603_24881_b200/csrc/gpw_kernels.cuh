@@ -1,0 +1,39 @@
+// Declarations shared by the CUDA translation units (collocate.cu, integrate.cu, gpw_api.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "gpw_math.cuh"
+
+namespace gpw {
+
+// Kernel parameters: geometry and per-level lists (lives in the constant bank).
+struct GridParams {
+    LevelGeom lev[GPW_MAX_LEVEL];
+    const long long *tile_base[GPW_MAX_LEVEL];   // collocation: per block, start of its visit list
+    const unsigned *seg[GPW_MAX_LEVEL];          // collocation: per block, start of each L segment
+    const long long *brick_base[GPW_MAX_LEVEL];  // integration: per brick, start of its entry list
+    double *grid[GPW_MAX_LEVEL];                 // rho (written) or v (read)
+};
+
+// Pair record as the kernels use it, loaded with three 16-byte loads.
+struct PairRec {
+    double nP0, nP1, nP2, ap, cc;
+    long long coef_off;
+};
+
+__device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, int task) {
+    const double2 *tk = reinterpret_cast<const double2 *>(tasks + task);
+    const double2 a = __ldg(tk), b = __ldg(tk + 1), d = __ldg(tk + 2);
+    PairRec r;
+    r.nP0 = a.x; r.nP1 = a.y; r.nP2 = b.x; r.ap = b.y; r.cc = d.x;
+    r.coef_off = __double_as_longlong(d.y);
+    return r;
+}
+
+// launchers (each picks the instantiation for the plan's largest L)
+cudaError_t launch_collocate(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items,
+                             int nitem, const double *coef, int deriv, int max_L, cudaStream_t st);
+cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
+                             int nitem, double *mom, int deriv, int max_L, cudaStream_t st);
+
+}  // namespace gpw

@@ -106,6 +106,14 @@ void build_S(const double *H, std::vector<double> &S) {
     }
 }
 
+struct RawEntry {
+    long long key;  // global brick id (level-major)
+    int task;
+    signed char s[3];
+    unsigned char L;
+    unsigned mask;
+};
+
 struct RawVisit {
     long long key;  // global block id (level-major)
     int task;
@@ -190,6 +198,8 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
             g.ecut = e;
             g.ntile = g.T[0] * g.T[1] * g.T[2];
+            for (int i = 0; i < 3; i++) g.B[i] = (g.T[i] + BRICK - 1) / BRICK;
+            g.nbrick = g.B[0] * g.B[1] * g.B[2];
             g.dV = hp->omega / ((double)g.N[0] * g.N[1] * g.N[2]);
             for (int c = 0; c < 3; c++)
                 for (int i = 0; i < 3; i++) {
@@ -317,6 +327,9 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         std::vector<long long> lev_tile0(nlevel + 1, 0);
         for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;
         const long long ntile_all = lev_tile0[nlevel];
+        std::vector<long long> lev_brick0(nlevel + 1, 0);
+        for (int a = 0; a < nlevel; a++) lev_brick0[a + 1] = lev_brick0[a] + hp->lev[a].nbrick;
+        const long long nbrick_all = lev_brick0[nlevel];
         // circumradius of a block about its centre (points at +-1.5 steps per axis)
         std::vector<double> circ(nlevel);
         for (int a = 0; a < nlevel; a++) {
@@ -332,10 +345,13 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         const long chunk = 256;
         const long nchunk = (ntask + chunk - 1) / chunk;
         std::vector<std::vector<RawVisit>> raw(nchunk);
+        std::vector<std::vector<RawEntry>> rawb(nchunk);
         std::atomic<int> wrap_overflow(0);
         parallel_chunks(ntask, chunk, nthread, [&](long c, long lo, long hi, int) {
             std::vector<RawVisit> &rv = raw[c];
+            std::vector<RawEntry> &rb = rawb[c];
             for (long ti = lo; ti < hi; ti++) {
+                const size_t rb0 = rb.size();   // this pair's entries start here
                 const HostTask &t = hp->task[ti];
                 const LevelGeom &g = hp->lev[t.level];
                 const int *N = g.N;
@@ -389,6 +405,20 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                             v.s[0] = (signed char)s1; v.s[1] = (signed char)s2; v.s[2] = (signed char)s3;
                             v.L = (unsigned char)(t.la + t.lb);
                             rv.push_back(v);
+                            // the same visit in the brick lists of the integration kernel
+                            const long long bkey = lev_brick0[t.level] +
+                                ((long long)(w1 / BRICK) * g.B[1] + (w2 / BRICK)) * g.B[2] + (w3 / BRICK);
+                            const unsigned bit = 1u << (((w1 % BRICK) * BRICK + (w2 % BRICK)) * BRICK + (w3 % BRICK));
+                            size_t e = rb0;
+                            for (; e < rb.size(); e++)
+                                if (rb[e].key == bkey && rb[e].s[0] == v.s[0] && rb[e].s[1] == v.s[1] && rb[e].s[2] == v.s[2]) break;
+                            if (e == rb.size()) {
+                                RawEntry ne;
+                                ne.key = bkey; ne.task = (int)ti; ne.L = v.L; ne.mask = 0;
+                                ne.s[0] = v.s[0]; ne.s[1] = v.s[1]; ne.s[2] = v.s[2];
+                                rb.push_back(ne);
+                            }
+                            rb[e].mask |= bit;
                         }
             }
         });
@@ -431,6 +461,54 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                     acc += segcnt[(size_t)(lev_tile0[a] + tl) * 8 + L];
                 }
             }
+        }
+        // ---- brick lists of the integration kernel (counting sort by brick, pair order kept) ----
+        {
+            std::vector<long long> bcnt(nbrick_all + 1, 0);
+            long long nent = 0;
+            for (auto &rb : rawb) {
+                nent += (long long)rb.size();
+                for (const RawEntry &e : rb) bcnt[e.key + 1]++;
+            }
+            for (long long i = 0; i < nbrick_all; i++) bcnt[i + 1] += bcnt[i];
+            hp->bentry.resize((size_t)nent);
+            std::vector<long long> cur(bcnt.begin(), bcnt.end() - 1);
+            for (auto &rb : rawb) {
+                for (const RawEntry &e : rb) {
+                    BEntry &o = hp->bentry[(size_t)cur[e.key]++];
+                    o.task = e.task; o.s[0] = e.s[0]; o.s[1] = e.s[1]; o.s[2] = e.s[2]; o.L = e.L; o.mask = e.mask; o.pad = 0;
+                    hp->max_L = std::max(hp->max_L, (int)e.L);
+                }
+                std::vector<RawEntry>().swap(rb);
+            }
+            hp->brick_base.resize(nlevel);
+            const unsigned BITEM_MAX = 768;
+            std::vector<std::pair<long long, BItem>> tmp;
+            for (int a = 0; a < nlevel; a++) {
+                const int nb = hp->lev[a].nbrick;
+                hp->brick_base[a].assign(bcnt.begin() + lev_brick0[a], bcnt.begin() + lev_brick0[a] + nb + 1);
+                for (int b = 0; b < nb; b++) {
+                    const long long base = hp->brick_base[a][b];
+                    const unsigned n = (unsigned)(hp->brick_base[a][b + 1] - base);
+                    if (!n) continue;
+                    const unsigned nparts = (n + BITEM_MAX - 1) / BITEM_MAX;
+                    for (unsigned p = 0; p < nparts; p++) {
+                        BItem it;
+                        it.level = a; it.brick = b;
+                        it.lo = (unsigned)((unsigned long long)n * p / nparts);
+                        it.hi = (unsigned)((unsigned long long)n * (p + 1) / nparts);
+                        long long work = 0;
+                        for (unsigned e = it.lo; e < it.hi; e++) {
+                            const BEntry &be = hp->bentry[(size_t)(base + e)];
+                            work += (long long)__builtin_popcount(be.mask) * (4 + be.L);
+                        }
+                        tmp.emplace_back(work, it);
+                    }
+                }
+            }
+            std::stable_sort(tmp.begin(), tmp.end(), [](const std::pair<long long, BItem> &x, const std::pair<long long, BItem> &y) { return x.first > y.first; });
+            hp->bitem.reserve(tmp.size());
+            for (auto &x : tmp) hp->bitem.push_back(x.second);
         }
         // ---- work items: every block's list cut into ranges of at most ITEM_MAX visits ----
         const unsigned ITEM_MAX = 384;
