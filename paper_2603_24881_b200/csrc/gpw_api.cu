@@ -130,6 +130,7 @@ void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
         P.seg[a] = p->d_seg[a];
         P.brick_base[a] = p->d_brick_base[a];
         P.grid[a] = grids[a];
+        for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[a][L];
     }
 }
 

@@ -43,14 +43,15 @@ struct LevelGeom {
     double ecut;     // E_alpha of T5
 };
 
-// Pair record read by the collocation / integration kernels (48 bytes, three 16-byte loads).
+// Pair record read by the collocation / integration kernels (64 bytes, four 16-byte loads).
 struct TaskK {
     double nP[3];        // Gaussian-product centre P in grid-index units of its level
     double ap;           // a_p = a_a + a_b
-    double cc;           // exp(-2 a_p Gm33): second-order ratio of the Gaussian recursion along n3 (Eq. 25)
+    double c22, c23;     // exp(-2 a_p Gm22), exp(-2 a_p Gm23): second-order ratios of the Gaussian recursion
+    double c33;          // exp(-2 a_p Gm33)   (Eq. 25; the cross term is the integer-index reading of A.31-A.32)
     long long coef_off;  // offset (doubles) of the pair's polynomial / moment vector in the workspace
 };
-static_assert(sizeof(TaskK) == 48, "TaskK must be 48 bytes");
+static_assert(sizeof(TaskK) == 64, "TaskK must be 64 bytes");
 
 // Pair record read by the pre-pass (D block -> polynomial) and post-pass (moments -> F block).
 struct TaskP {
@@ -119,14 +120,19 @@ struct HostPlan {
     std::vector<TaskK> taskK;
     std::vector<TaskP> taskP;
     long long ncoef_total = 0;
+    // workspace offset of pair i of class (level, L) = coef_base[level][L] + i * ncoef_pad(L)
+    long long coef_base[GPW_MAX_LEVEL][NLSEG + 1] = {{0}};
+    bool coef_base_set[GPW_MAX_LEVEL][NLSEG + 1] = {{false}};
     // per level block lists
     std::vector<std::vector<long long>> tile_base;   // [level][ntile+1] global visit index
     std::vector<std::vector<unsigned>> seg;          // [level][ntile*8] start of each L segment (relative)
     std::vector<Visit> visit;                        // all levels, level-major, block-major
     std::vector<Item> item;                          // sorted by descending size
     std::vector<std::vector<long long>> brick_base;  // [level][nbrick+1] global entry index
-    std::vector<BEntry> bentry;                      // all levels, level-major, brick-major, sorted by L
+    std::vector<BEntry> bentry;                      // all levels, level-major, brick-major; inside a brick by L,
+                                                     // inside an L segment by decreasing number of visited blocks
     std::vector<BItem> bitem;                        // sorted by descending work
+    std::vector<std::vector<unsigned>> bseg;         // [level][nbrick*8] start of each L segment (relative)
     int max_L = 0;                                   // largest la + lb present
     long nvisit_level[GPW_MAX_LEVEL] = {0};
     long ntask_level[GPW_MAX_LEVEL] = {0};

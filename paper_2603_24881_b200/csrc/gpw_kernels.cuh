@@ -13,19 +13,20 @@ struct GridParams {
     const unsigned *seg[GPW_MAX_LEVEL];          // collocation: per block, start of each L segment
     const long long *brick_base[GPW_MAX_LEVEL];  // integration: per brick, start of its entry list
     double *grid[GPW_MAX_LEVEL];                 // rho (written) or v (read)
+    long long coef_base[GPW_MAX_LEVEL][8];       // workspace offset of pair i of class (level, L) = base + i * ncoef_pad(L)
 };
 
-// Pair record as the kernels use it, loaded with three 16-byte loads.
+// Pair record as the kernels use it, loaded with four 16-byte loads.
 struct PairRec {
-    double nP0, nP1, nP2, ap, cc;
+    double nP0, nP1, nP2, ap, c22, c23, c33;
     long long coef_off;
 };
 
 __device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, int task) {
     const double2 *tk = reinterpret_cast<const double2 *>(tasks + task);
-    const double2 a = __ldg(tk), b = __ldg(tk + 1), d = __ldg(tk + 2);
+    const double2 a = __ldg(tk), b = __ldg(tk + 1), c = __ldg(tk + 2), d = __ldg(tk + 3);
     PairRec r;
-    r.nP0 = a.x; r.nP1 = a.y; r.nP2 = b.x; r.ap = b.y; r.cc = d.x;
+    r.nP0 = a.x; r.nP1 = a.y; r.nP2 = b.x; r.ap = b.y; r.c22 = c.x; r.c23 = c.y; r.c33 = d.x;
     r.coef_off = __double_as_longlong(d.y);
     return r;
 }

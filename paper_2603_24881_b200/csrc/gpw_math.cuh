@@ -211,6 +211,206 @@ GPW_HD void colloc_column(const double *__restrict__ c, const double *q, double 
     }
 }
 
+// ------------------------------------------------------------------------------------------ slab form
+// A lane owns the slab of 4 x 4 grid points (rows j along n2, points t along n3) at its own n1.  The
+// polynomial is collapsed once per slab in u1 (b[ky][kz]), once per row in u2 (a[kz]) and swept by Horner
+// in u3 per point; the Gaussian is one exp() at the slab corner plus two first-step ratios, everything
+// else follows by the recursion of Eq. (24)-(25) with the constant second-order ratios c22, c23, c33.
+
+// number of (ky,kz) with ky + kz <= L, and the position of (ky,kz) among them (kz-major)
+GPW_HD constexpr int npair2(int L) { return L < 0 ? 0 : (L + 1) * (L + 2) / 2; }
+GPW_HD constexpr int bidx(int L, int ky, int kz) {
+    int o = 0;
+    for (int z = 0; z < kz; z++) o += L - z + 1;
+    return o + ky;
+}
+
+// Gaussian at the slab corner and the first-step ratios along n2 and n3.
+//   g0 = exp(-E(u1,u20,u30)),  r2 = G(j=1,t=0)/G(0,0),  r3 = G(0,1)/G(0,0)
+// Every intermediate of the recursion is a true Gaussian value or a true ratio of neighbouring values; the
+// plan builder routes pairs for which one of them could leave the FP64 range (pairs far sharper than their
+// grid resolves, reading A23) to the direct class instead (plan.cpp, "direct class").
+struct SlabGauss { double g0, r2, r3; };
+GPW_HD SlabGauss slab_gauss(const double *q, double u1, double u20, double u30) {
+    const double E0 = q[0] * u1 * u1 + q[1] * u20 * u20 + q[2] * u30 * u30 +
+                      2.0 * (q[3] * u1 * u20 + (q[4] * u1 + q[5] * u20) * u30);
+    const double s2 = 2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30) + q[1];
+    const double s3 = 2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30) + q[2];
+    SlabGauss G;
+    G.g0 = exp(-E0); G.r2 = exp(-s2); G.r3 = exp(-s3);
+    return G;
+}
+GPW_HD double gauss_direct(const double *q, double u1, double u2, double u3) {
+    return exp(-(q[0] * u1 * u1 + q[1] * u2 * u2 + q[2] * u3 * u3 +
+                 2.0 * (q[3] * u1 * u2 + (q[4] * u1 + q[5] * u2) * u3)));
+}
+
+// Collocation of one pair on one slab.  acc[NCOMP][16] (index j*4+t); for DERIV the gradient is
+// accumulated in grid-index (covariant) components.
+template <int L, int DERIV>
+GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c22, double c23, double c33,
+                        double u1, double u20, double u30, double (*acc)[16]) {
+    constexpr int NB = npair2(L), NBX = npair2(L - 1);
+    double b[NB], bx[NBX > 0 ? NBX : 1];
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+        for (int ky = 0; ky <= L - kz; ky++) {
+            double p = 0.0, dp = 0.0;
+#pragma unroll
+            for (int kx = L - kz - ky; kx >= 0; kx--) {
+                if (DERIV) dp = dp * u1 + p;
+                p = p * u1 + c[cidx(L, kx, ky, kz)];
+            }
+            b[bidx(L, ky, kz)] = p;
+            if (DERIV && ky + kz <= L - 1) bx[bidx(L - 1, ky, kz)] = dp;
+        }
+    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+    double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
+    // -2 (q u)_i at the row start, its step per row and per point
+    double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
+    if (DERIV) {
+        qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
+        qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
+        qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const double u2 = u20 + j;
+        double a[L + 1], ax[L > 0 ? L : 1], ay[L > 0 ? L : 1];
+#pragma unroll
+        for (int kz = 0; kz <= L; kz++) {
+            double s = 0.0, sy = 0.0;
+#pragma unroll
+            for (int ky = L - kz; ky >= 0; ky--) {
+                if (DERIV) sy = sy * u2 + s;
+                s = s * u2 + b[bidx(L, ky, kz)];
+            }
+            a[kz] = s;
+            if (DERIV && kz < L) {
+                ay[kz] = sy;
+                double sx = 0.0;
+#pragma unroll
+                for (int ky = L - 1 - kz; ky >= 0; ky--) sx = sx * u2 + bx[bidx(L - 1, ky, kz)];
+                ax[kz] = sx;
+            }
+        }
+        double g = grow, r = r3row;
+        double p1 = qr1, p2 = qr2, p3 = qr3;
+#pragma unroll
+        for (int t = 0; t < 4; t++) {
+            const double u3 = u30 + t;
+            double Q = 0.0, Qz = 0.0;
+#pragma unroll
+            for (int kz = L; kz >= 0; kz--) {
+                if (DERIV) Qz = Qz * u3 + Q;
+                Q = Q * u3 + a[kz];
+            }
+            const double w = g * Q;
+            acc[0][j * 4 + t] += w;
+            if constexpr (DERIV != 0) {
+                double Qx = 0.0, Qy = 0.0;
+#pragma unroll
+                for (int kz = L - 1; kz >= 0; kz--) { Qx = Qx * u3 + ax[kz]; Qy = Qy * u3 + ay[kz]; }
+                acc[1][j * 4 + t] += g * Qx + w * p1;
+                acc[2][j * 4 + t] += g * Qy + w * p2;
+                acc[3][j * 4 + t] += g * Qz + w * p3;
+                p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
+            }
+            g *= r; r *= c33;
+        }
+        grow *= r2; r2 *= c22; r3row *= c23;
+        if (DERIV) { qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5]; }
+    }
+}
+
+// Integration of one pair on one slab (exact transpose of colloc_slab).
+//   v   [NCOMP][16] (index j*4+t): v0 and, for DERIV, the vector field in grid-index (contravariant)
+//       components z'_i = sum_c Hinv[i][c] w_c
+//   m   the lane's private moment vector (cidx order), accumulated
+template <int L, int DERIV>
+GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, double c23, double c33, double u1,
+                       double u20, double u30, double *m) {
+    constexpr int NB = npair2(L), NBX = npair2(L - 1);
+    double B0[NB], B1[NBX > 0 ? NBX : 1];
+#pragma unroll
+    for (int i = 0; i < NB; i++) B0[i] = 0.0;
+#pragma unroll
+    for (int i = 0; i < NBX; i++) B1[i] = 0.0;
+    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+    double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
+    double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
+    if (DERIV) {
+        qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
+        qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
+        qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const double u2 = u20 + j;
+        double A0[L + 1], A1[L > 0 ? L : 1], A2[L > 0 ? L : 1], A3[L > 0 ? L : 1];
+#pragma unroll
+        for (int kz = 0; kz <= L; kz++) A0[kz] = 0.0;
+#pragma unroll
+        for (int kz = 0; kz < L; kz++) { A1[kz] = 0.0; A2[kz] = 0.0; A3[kz] = 0.0; }
+        double g = grow, r = r3row;
+        double p1 = qr1, p2 = qr2, p3 = qr3;
+#pragma unroll
+        for (int t = 0; t < 4; t++) {
+            const double u3 = u30 + t;
+            double g0 = v[0][j * 4 + t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
+            if constexpr (DERIV != 0) {
+                const double z1 = v[1][j * 4 + t], z2 = v[2][j * 4 + t], z3 = v[3][j * 4 + t];
+                g0 += z1 * p1 + z2 * p2 + z3 * p3;
+                g1 = g * z1; g2 = g * z2; g3 = g * z3;
+                p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
+            }
+            g0 *= g;
+            double pw = 1.0;
+#pragma unroll
+            for (int kz = 0; kz <= L; kz++) {
+                A0[kz] += g0 * pw;
+                if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
+                if (kz < L) pw *= u3;
+            }
+            g *= r; r *= c33;
+        }
+        grow *= r2; r2 *= c22; r3row *= c23;
+        if (DERIV) {
+            qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5];
+#pragma unroll
+            for (int kz = 1; kz <= L; kz++) A0[kz] += kz * A3[kz - 1];
+        }
+        double pw2[L + 1];
+        pw2[0] = 1.0;
+#pragma unroll
+        for (int k = 1; k <= L; k++) pw2[k] = pw2[k - 1] * u2;
+#pragma unroll
+        for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+            for (int ky = 0; ky <= L - kz; ky++) {
+                double s = A0[kz] * pw2[ky];
+                if (DERIV && ky > 0) s += A2[kz] * (ky * pw2[ky - 1]);
+                B0[bidx(L, ky, kz)] += s;
+                if (DERIV && ky + kz <= L - 1) B1[bidx(L - 1, ky, kz)] += A1[kz] * pw2[ky];
+            }
+    }
+    double pw1[L + 1];
+    pw1[0] = 1.0;
+#pragma unroll
+    for (int k = 1; k <= L; k++) pw1[k] = pw1[k - 1] * u1;
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+        for (int ky = 0; ky <= L - kz; ky++)
+#pragma unroll
+            for (int kx = 0; kx <= L - kz - ky; kx++) {
+                double s = B0[bidx(L, ky, kz)] * pw1[kx];
+                if (DERIV && kx > 0) s += B1[bidx(L - 1, ky, kz)] * (kx * pw1[kx - 1]);
+                m[cidx(L, kx, ky, kz)] += s;
+            }
+}
+
 // Integration of one pair on one column of four points (transpose of colloc_column).
 //   v      [NCOMP][4]: v0 and, for DERIV, the vector field already mapped to grid-index coordinates
 //   m      the thread's private moment vector (cidx order), accumulated

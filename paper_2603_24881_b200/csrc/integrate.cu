@@ -91,7 +91,7 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
                 const double2 x1 = *reinterpret_cast<const double2 *>(vb + k * 64 + 32);
                 vv[k][0] = x0.x; vv[k][1] = x0.y; vv[k][2] = x1.x; vv[k][3] = x1.y;
             }
-            integ_column<L, DERIV>(vv, q, pr.cc, u1b + 4 * t1, u2b + 4 * t2, u3b + 4 * t3, m);
+            integ_column<L, DERIV>(vv, q, pr.c33, u1b + 4 * t1, u2b + 4 * t2, u3b + 4 * t3, m);
         }
     }
     int off = 0, cnt = NC;

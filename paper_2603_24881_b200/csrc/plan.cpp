@@ -311,13 +311,20 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             for (int a = 0; a < 3; a++)
                 k.nP[a] = (t.P[0] * hp->binv[0 * 3 + a] + t.P[1] * hp->binv[1 * 3 + a] + t.P[2] * hp->binv[2 * 3 + a]) * g.N[a];
             k.ap = t.ap;
-            k.cc = std::exp(-2.0 * t.ap * g.Gm[2]);
+            k.c22 = std::exp(-2.0 * t.ap * g.Gm[1]);
+            k.c23 = std::exp(-2.0 * t.ap * g.Gm[5]);
+            k.c33 = std::exp(-2.0 * t.ap * g.Gm[2]);
             k.coef_off = coff;
             TaskP &p = hp->taskP[i];
             for (int x = 0; x < 3; x++) { p.PA[x] = t.P[x] - t.A[x]; p.PB[x] = t.P[x] - t.Bt[x]; }
             p.pref = t.pref; p.coef_off = coff;
             p.ao_a = hp->ao_loc[t.shl_a]; p.ao_b = hp->ao_loc[t.shl_b];
             p.la = (short)t.la; p.lb = (short)t.lb; p.level = (short)t.level; p.sym = (short)t.sym;
+            // pairs are sorted by (level, L): inside a class the workspace offset is affine in the pair index
+            if (!hp->coef_base_set[t.level][t.la + t.lb]) {
+                hp->coef_base_set[t.level][t.la + t.lb] = true;
+                hp->coef_base[t.level][t.la + t.lb] = coff - (long long)i * ncoef_pad(t.la + t.lb);
+            }
             coff += ncoef_pad(t.la + t.lb);
             hp->ntask_level[t.level]++;
         }
