@@ -19,8 +19,11 @@ constexpr int MAXL = GPW_MAX_L;          // shells up to f
 constexpr int MAXLP = 2 * MAXL;          // pair polynomial degree L = la + lb <= 6
 constexpr int NLSEG = MAXLP + 1;         // visit lists are segmented by L = 0..6
 constexpr int TILE = 4;                  // grid block edge
-constexpr int BRICK = 3;                 // integration stages bricks of BRICK^3 grid blocks in shared memory
-constexpr int BRICK_TILES = BRICK * BRICK * BRICK;
+// integration stages bricks of BR1 x BR2 x BR3 grid blocks in shared memory; one block thick along n1 so
+// that a lane (which owns one n1 plane of a block) keeps the same u1 for every block of a brick entry
+constexpr int BR1 = 1, BR2 = 5, BR3 = 5;
+constexpr int BRICK_TILES = BR1 * BR2 * BR3;
+static_assert(BR1 == 1 && BRICK_TILES <= 32, "brick: one block along n1, mask of at most 32 blocks");
 
 // number of monomials u1^kx u2^ky u3^kz with kx+ky+kz <= L
 GPW_CX int ncoef(int L) { return (L + 1) * (L + 2) * (L + 3) / 6; }
@@ -34,7 +37,7 @@ struct LevelGeom {
     int T[3];        // 4x4x4 blocks per axis
     int ntile;       // T[0]*T[1]*T[2]
     int nbrick;      // B[0]*B[1]*B[2]
-    int B[3];        // bricks per axis, ceil(T / BRICK) (the last brick of an axis may be ragged)
+    int B[3];        // bricks per axis, ceil(T_i / BR_i) (the last brick of an axis may be ragged)
     int pad0;
     double H[9];     // H[c*3+i] = component c of the grid step vector a_i / N_i :  r - P = H (n - n_P)
     double Hinv[9];  // Hinv[i*3+c]:  u_i = sum_c Hinv[i*3+c] X_c
@@ -87,7 +90,7 @@ struct BEntry {
     int task;
     signed char s[3];     // lattice wraps of this image
     unsigned char L;      // la + lb
-    unsigned mask;        // bit ((t1*BRICK + t2)*BRICK + t3) set: block (t1,t2,t3) of the brick is visited
+    unsigned mask;        // bit (t2*BR3 + t3) set: block (t2,t3) of the brick is visited
     unsigned pad;
 };
 static_assert(sizeof(BEntry) == 16, "BEntry must be 16 bytes");
@@ -96,8 +99,12 @@ static_assert(sizeof(BEntry) == 16, "BEntry must be 16 bytes");
 struct BItem {
     int level;
     int brick;
+    long long base;       // global index of the brick's first entry
     unsigned lo, hi;      // entry range relative to the brick's list
+    unsigned seg[8];      // start of each L segment of the brick's list (relative); seg[7] = list length
+    unsigned pad[2];
 };
+static_assert(sizeof(BItem) == 64, "BItem must be 64 bytes");
 
 struct HostTask {
     int shl_a, prim_a, shl_b, prim_b;
@@ -132,7 +139,6 @@ struct HostPlan {
     std::vector<BEntry> bentry;                      // all levels, level-major, brick-major; inside a brick by L,
                                                      // inside an L segment by decreasing number of visited blocks
     std::vector<BItem> bitem;                        // sorted by descending work
-    std::vector<std::vector<unsigned>> bseg;         // [level][nbrick*8] start of each L segment (relative)
     int max_L = 0;                                   // largest la + lb present
     long nvisit_level[GPW_MAX_LEVEL] = {0};
     long ntask_level[GPW_MAX_LEVEL] = {0};

@@ -324,20 +324,21 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
     }
 }
 
-// Integration of one pair on one slab (exact transpose of colloc_slab).
-//   v   [NCOMP][16] (index j*4+t): v0 and, for DERIV, the vector field in grid-index (contravariant)
-//       components z'_i = sum_c Hinv[i][c] w_c
-//   m   the lane's private moment vector (cidx order), accumulated
-template <int L, int DERIV>
-GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, double c23, double c33, double u1,
-                       double u20, double u30, double *m) {
-    constexpr int NB = npair2(L), NBX = npair2(L - 1);
-    double B0[NB], B1[NBX > 0 ? NBX : 1];
-#pragma unroll
-    for (int i = 0; i < NB; i++) B0[i] = 0.0;
-#pragma unroll
-    for (int i = 0; i < NBX; i++) B1[i] = 0.0;
-    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+// Integration of one pair on one slab (exact transpose of colloc_slab), in two parts.
+//
+// integ_slab_rows: the u3 and u2 sweeps.  Accumulates the slab's partial moments at fixed u1,
+//     B0[bidx(L,ky,kz)]   += sum_{j,t} g (v0 + z . p) u2^ky u3^kz   + derivative terms in u2, u3
+//     B1[bidx(L-1,ky,kz)] += sum_{j,t} g z1 u2^ky u3^kz              (DERIV; multiplies d/du1)
+// with p = -2 (q u) (the Gaussian's logarithmic gradient) and z the vector field in grid-index
+// (contravariant) components.  vrow(comp, j, out[4]) delivers the four values of row j of component comp.
+// A lane of the integration kernel keeps B0 / B1 over ALL blocks of a brick entry: the brick is one block
+// thick along n1, so the lane's u1 is the same for every block.
+//
+// integ_expand_u1: m[cidx(L,kx,ky,kz)] (+)= B0 u1^kx + kx u1^(kx-1) B1 -- once per entry.
+template <int L, int DERIV, class VRow>
+GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23, double c33,
+                            const SlabGauss SG, double u1, double u20, double u30, double *B0, double *B1) {
+    constexpr int NCOMP = DERIV ? 4 : 1;
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
     if (DERIV) {
@@ -348,6 +349,9 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
 #pragma unroll
     for (int j = 0; j < 4; j++) {
         const double u2 = u20 + j;
+        double vv[NCOMP][4];
+#pragma unroll
+        for (int k = 0; k < NCOMP; k++) vrow(k, j, vv[k]);
         double A0[L + 1], A1[L > 0 ? L : 1], A2[L > 0 ? L : 1], A3[L > 0 ? L : 1];
 #pragma unroll
         for (int kz = 0; kz <= L; kz++) A0[kz] = 0.0;
@@ -358,9 +362,9 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
 #pragma unroll
         for (int t = 0; t < 4; t++) {
             const double u3 = u30 + t;
-            double g0 = v[0][j * 4 + t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
+            double g0 = vv[0][t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
             if constexpr (DERIV != 0) {
-                const double z1 = v[1][j * 4 + t], z2 = v[2][j * 4 + t], z3 = v[3][j * 4 + t];
+                const double z1 = vv[1][t], z2 = vv[2][t], z3 = vv[3][t];
                 g0 += z1 * p1 + z2 * p2 + z3 * p3;
                 g1 = g * z1; g2 = g * z2; g3 = g * z3;
                 p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
@@ -369,9 +373,14 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
             double pw = 1.0;
 #pragma unroll
             for (int kz = 0; kz <= L; kz++) {
-                A0[kz] += g0 * pw;
-                if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
-                if (kz < L) pw *= u3;
+                if (kz == 0) {
+                    A0[0] += g0;
+                    if (DERIV && L > 0) { A1[0] += g1; A2[0] += g2; A3[0] += g3; }
+                } else {
+                    A0[kz] += g0 * pw;
+                    if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
+                }
+                if (kz < L) pw = kz == 0 ? u3 : pw * u3;
             }
             g *= r; r *= c33;
         }
@@ -384,17 +393,43 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
         double pw2[L + 1];
         pw2[0] = 1.0;
 #pragma unroll
-        for (int k = 1; k <= L; k++) pw2[k] = pw2[k - 1] * u2;
+        for (int k = 1; k <= L; k++) pw2[k] = k == 1 ? u2 : pw2[k - 1] * u2;
 #pragma unroll
         for (int kz = 0; kz <= L; kz++)
 #pragma unroll
             for (int ky = 0; ky <= L - kz; ky++) {
-                double s = A0[kz] * pw2[ky];
-                if (DERIV && ky > 0) s += A2[kz] * (ky * pw2[ky - 1]);
-                B0[bidx(L, ky, kz)] += s;
-                if (DERIV && ky + kz <= L - 1) B1[bidx(L - 1, ky, kz)] += A1[kz] * pw2[ky];
+                if (ky == 0) B0[bidx(L, 0, kz)] += A0[kz];
+                else B0[bidx(L, ky, kz)] += A0[kz] * pw2[ky];
+                if (DERIV && ky > 0) B0[bidx(L, ky, kz)] += A2[kz] * (ky * pw2[ky - 1]);
+                if (DERIV && ky + kz <= L - 1) {
+                    if (ky == 0) B1[bidx(L - 1, 0, kz)] += A1[kz];
+                    else B1[bidx(L - 1, ky, kz)] += A1[kz] * pw2[ky];
+                }
             }
     }
+}
+
+// contribution of this lane's B0 / B1 to moment (kx,ky,kz):  B0 u1^kx + kx u1^(kx-1) B1
+template <int L, int DERIV>
+GPW_HD double integ_expand_term(const double *B0, const double *B1, const double *pw1, int kx, int ky, int kz) {
+    double s = kx == 0 ? B0[bidx(L, ky, kz)] : B0[bidx(L, ky, kz)] * pw1[kx];
+    if (DERIV && kx > 0) s += B1[bidx(L - 1, ky, kz)] * (kx * pw1[kx - 1]);
+    return s;
+}
+
+template <int L, int DERIV>
+GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, double c23, double c33, double u1,
+                       double u20, double u30, double *m) {
+    constexpr int NB = npair2(L), NBX = npair2(L - 1);
+    double B0[NB], B1[NBX > 0 ? NBX : 1];
+#pragma unroll
+    for (int i = 0; i < NB; i++) B0[i] = 0.0;
+#pragma unroll
+    for (int i = 0; i < NBX; i++) B1[i] = 0.0;
+    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+    integ_slab_rows<L, DERIV>([&](int k, int j, double *o) {
+        for (int t = 0; t < 4; t++) o[t] = v[k][j * 4 + t];
+    }, q, c22, c23, c33, SG, u1, u20, u30, B0, B1);
     double pw1[L + 1];
     pw1[0] = 1.0;
 #pragma unroll
@@ -404,11 +439,8 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
 #pragma unroll
         for (int ky = 0; ky <= L - kz; ky++)
 #pragma unroll
-            for (int kx = 0; kx <= L - kz - ky; kx++) {
-                double s = B0[bidx(L, ky, kz)] * pw1[kx];
-                if (DERIV && kx > 0) s += B1[bidx(L - 1, ky, kz)] * (kx * pw1[kx - 1]);
-                m[cidx(L, kx, ky, kz)] += s;
-            }
+            for (int kx = 0; kx <= L - kz - ky; kx++)
+                m[cidx(L, kx, ky, kz)] += integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
 }
 
 // Integration of one pair on one column of four points (transpose of colloc_column).

@@ -1,128 +1,116 @@
 // Integration kernel (Eq. 4 with the quadrature of Eq. 29; the work of Alg. 2,
 // PAPER.md:240-263, re-decomposed for B200).
 //
-// One CTA per work item = one brick of 3x3x3 grid blocks and a range of its entry list; an entry is a
+// One CTA per work item = one brick of 1 x 5 x 5 grid blocks and a range of its entry list; an entry is a
 // (pair, lattice image) with the mask of the brick's blocks it visits.  The CTA stages the brick of v in
-// shared memory once (for DERIV with the vector field already mapped to grid-index components).  Each
-// warp then takes entries: per visited block a half-warp works with a lane per column of 4 points,
-// accumulating the pair's moment vector m[k] = sum_r w(r) G(r) u^k in private registers over ALL the
-// entry's blocks; one shuffle reduce-scatter over the warp and one atomic add per moment finish the
-// entry.  Alg. 2 instead adds nca*ncb values per (pair, block) to global memory;
-// amortising over the brick cuts that traffic by the blocks per entry.
+// shared memory once (for DERIV with the vector field already mapped to grid-index components), laid out
+// per block and n1 plane.  A warp is eight groups of four lanes; a group owns one entry at a time and a
+// lane owns the n1 plane x of every block, i.e. slabs of 4 x 4 points at a fixed u1.  Over all the
+// entry's blocks the lane accumulates the partial moments B0[ky][kz] (and B1 for DERIV) in registers
+// (gpw_math.cuh, integ_slab_rows); the expansion in u1, a shuffle reduction over the group's four lanes
+// and one FP64 atomic per moment finish the entry.  Alg. 2 instead adds nca*ncb values per (pair, block)
+// to global memory; amortising over the brick cuts that traffic by the blocks per
+// entry, and the moment form keeps the per-lane state at (L+1)(L+2)/2 doubles instead of nca*ncb.
 #include "gpw_kernels.cuh"
 
 namespace gpw {
 namespace {
 
 constexpr int NWARP = 4;
+constexpr int NGRP = 8;   // groups of 4 lanes per warp
 
-// ---- full-warp reduce-scatter of an N-vector with per-step padding --------------------------------
-// After the call lane holds `final_len(N)` sums in m[0..); element i of them is total[off + i] and is
-// valid iff i < cnt.
-GPW_CX int rs_final_len(int n) {
-    for (int b = 0; b < 5; b++) n = n >= 2 ? (n + 1) / 2 : 1;
-    return n;
-}
-
-template <int LEN, int BIT>
-__device__ __forceinline__ void rs_step(double *m, int lane, int &off, int &cnt) {
-    if constexpr (BIT >= 1) {
-        const bool up = lane & BIT;
-        if constexpr (LEN >= 2) {
-            constexpr int HALF = (LEN + 1) / 2;
-#pragma unroll
-            for (int i = 0; i < HALF; i++) {
-                const double lo = m[i];
-                const double hi = (i + HALF < LEN) ? m[i + HALF] : 0.0;
-                const double send = up ? lo : hi;
-                const double keep = up ? hi : lo;
-                m[i] = keep + __shfl_xor_sync(0xffffffffu, send, BIT);
-            }
-            off += up ? HALF : 0;
-            cnt = up ? cnt - HALF : min(cnt, HALF);
-            rs_step<HALF, BIT / 2>(m, lane, off, cnt);
-        } else {
-            m[0] += __shfl_xor_sync(0xffffffffu, m[0], BIT);
-            if (up) cnt = 0;   // the partner with the bit clear owns the sum
-            rs_step<1, BIT / 2>(m, lane, off, cnt);
-        }
-    }
-}
+// shared-memory chunk = the 4 x 4 points of one n1 plane of one block, all components, plus 16 bytes of
+// padding: the four lanes of a group then read four different bank quarters with their 16-byte loads
+GPW_CX int chunk_doubles(int ncomp) { return ncomp * 16 + 2; }
 
 struct BrickCtx {
-    const TaskK *tasks;
-    const BEntry *entries;   // already offset to the brick's list
-    const double *vs;        // shared memory brick: [block][comp][64], in-block order h*32 + col*2 + e
-    double gm[6];
+    const double *vs;        // shared memory brick: chunk (block, x) at (block*4 + x) * chunk_doubles
+    const double *gm;        // the level's metric (constant bank)
     int o1, o2, o3;          // stored grid index of the brick origin
     int N0, N1, N2;
+    int x;                   // lane within the group = n1 plane
 };
 
 template <int L, int DERIV>
-__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const PairRec pr, int lane,
+__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const PairRec pr, bool valid,
                                             double *__restrict__ mom) {
     constexpr int NCOMP = DERIV ? 4 : 1;
-    constexpr int NC = ncoef(L);
-    const int half = lane >> 4, col = lane & 15;
+    constexpr int CHS = chunk_doubles(NCOMP);
+    constexpr int NB = npair2(L), NBX = npair2(L - 1);
+    double B0[NB], B1[NBX > 0 ? NBX : 1];
+#pragma unroll
+    for (int i = 0; i < NB; i++) B0[i] = 0.0;
+#pragma unroll
+    for (int i = 0; i < (NBX > 0 ? NBX : 1); i++) B1[i] = 0.0;
     double q[6];
 #pragma unroll
-    for (int x = 0; x < 6; x++) q[x] = pr.ap * c.gm[x];
-    // column position relative to P for block (0,0,0) of the brick
-    const double u1b = (double)(c.o1 + (col >> 2) + en.s[0] * c.N0) - pr.nP0;
-    const double u2b = (double)(c.o2 + (col & 3) + en.s[1] * c.N1) - pr.nP1;
+    for (int k = 0; k < 6; k++) q[k] = pr.ap * c.gm[k];
+    const double u1 = (double)(c.o1 + c.x + en.s[0] * c.N0) - pr.nP0;
+    const double u2b = (double)(c.o2 + en.s[1] * c.N1) - pr.nP1;
     const double u3b = (double)(c.o3 + en.s[2] * c.N2) - pr.nP2;
-    double m[NC];
-#pragma unroll
-    for (int i = 0; i < NC; i++) m[i] = 0.0;
-    unsigned mask = en.mask;
-    while (mask) {   // warp-uniform: two blocks per trip, one per half-warp
-        const int bit0 = __ffs(mask) - 1;
+    unsigned mask = valid ? en.mask : 0u;
+    while (mask) {   // group-uniform
+        const int bit = __ffs(mask) - 1;
         mask &= mask - 1;
-        int bit1 = -1;
-        if (mask) { bit1 = __ffs(mask) - 1; mask &= mask - 1; }
-        const int my = half ? bit1 : bit0;
-        if (my >= 0) {
-            const int t1 = my / (BRICK * BRICK), t2 = (my / BRICK) % BRICK, t3 = my % BRICK;
-            const double *vb = c.vs + (size_t)my * (NCOMP * 64) + col * 2;
-            double vv[NCOMP][4];
-#pragma unroll
-            for (int k = 0; k < NCOMP; k++) {
-                const double2 x0 = *reinterpret_cast<const double2 *>(vb + k * 64);
-                const double2 x1 = *reinterpret_cast<const double2 *>(vb + k * 64 + 32);
-                vv[k][0] = x0.x; vv[k][1] = x0.y; vv[k][2] = x1.x; vv[k][3] = x1.y;
-            }
-            integ_column<L, DERIV>(vv, q, pr.c33, u1b + 4 * t1, u2b + 4 * t2, u3b + 4 * t3, m);
-        }
+        const int t2 = bit / BR3, t3 = bit - t2 * BR3;
+        const double *chunk = c.vs + (bit * 4 + c.x) * CHS;
+        const double u20 = u2b + 4 * t2, u30 = u3b + 4 * t3;
+        const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+        integ_slab_rows<L, DERIV>(
+            [&](int k, int j, double *o) {
+                const double2 a = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4);
+                const double2 b = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4 + 2);
+                o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+            },
+            q, pr.c22, pr.c23, pr.c33, SG, u1, u20, u30, B0, B1);
     }
-    int off = 0, cnt = NC;
-    rs_step<NC, 16>(m, lane, off, cnt);
-    double *dst = mom + pr.coef_off + off;
+    __syncwarp();
+    // expansion in u1, sum over the group's four lanes (n1 planes), one atomic per moment
+    double pw1[L + 1];
+    pw1[0] = 1.0;
 #pragma unroll
-    for (int i = 0; i < rs_final_len(NC); i++)
-        if (i < cnt) atomicAdd(dst + i, m[i]);
+    for (int k = 1; k <= L; k++) pw1[k] = pw1[k - 1] * u1;
+    double *dst = mom + pr.coef_off;
+#pragma unroll
+    for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+        for (int ky = 0; ky <= L - kz; ky++)
+#pragma unroll
+            for (int kx = 0; kx <= L - kz - ky; kx++) {
+                double s = integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
+                s += __shfl_xor_sync(0xffffffffu, s, 1);
+                s += __shfl_xor_sync(0xffffffffu, s, 2);
+                const int k = cidx(L, kx, ky, kz);
+                if (valid && (k & 3) == c.x) atomicAdd(dst + k, s);
+            }
 }
 
 template <int DERIV, int LMAX>
-__global__ void __launch_bounds__(NWARP * 32) k_integrate(const __grid_constant__ GridParams P,
-                                                           const TaskK *__restrict__ tasks,
-                                                           const BEntry *__restrict__ entries,
-                                                           const BItem *__restrict__ items,
-                                                           double *__restrict__ mom) {
+__global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
+                                                                          const TaskK *__restrict__ tasks,
+                                                                          const BEntry *__restrict__ entries,
+                                                                          const BItem *__restrict__ items,
+                                                                          double *__restrict__ mom) {
     constexpr int NCOMP = DERIV ? 4 : 1;
-    extern __shared__ __align__(16) double vs[];   // [BRICK_TILES][NCOMP][64]
-    const BItem it = items[blockIdx.x];
-    const LevelGeom &g = P.lev[it.level];
-    const int B2 = g.B[2], B1 = g.B[1];
-    const int k3 = it.brick % B2, k2 = (it.brick / B2) % B1, k1 = it.brick / (B2 * B1);
+    constexpr int CHS = chunk_doubles(NCOMP);
+    extern __shared__ __align__(16) double vs[];   // [BRICK_TILES * 4] chunks
+    __shared__ unsigned s_seg[8];
+    const BItem *itp = items + blockIdx.x;
+    const int level = itp->level, brick = itp->brick;
+    const unsigned it_lo = itp->lo, it_hi = itp->hi;
+    const long long ebase = itp->base;
+    if (threadIdx.x < 8) s_seg[threadIdx.x] = itp->seg[threadIdx.x];
+    const LevelGeom &g = P.lev[level];
+    const int B2 = g.B[2], B1n = g.B[1];
+    const int k3 = brick % B2, k2 = (brick / B2) % B1n, k1 = brick / (B2 * B1n);
     const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
-    const double *vin = P.grid[it.level];
-    // ---- stage the brick: one column (4 points x NCOMP) per thread and trip ----
-    for (int cidx_ = threadIdx.x; cidx_ < BRICK_TILES * 16; cidx_ += NWARP * 32) {
-        const int lt = cidx_ >> 4, col = cidx_ & 15;
-        const int t1 = lt / (BRICK * BRICK), t2 = (lt / BRICK) % BRICK, t3 = lt % BRICK;
-        const int b1 = BRICK * k1 + t1, b2 = BRICK * k2 + t2, b3 = BRICK * k3 + t3;
-        if (b1 >= g.T[0] || b2 >= g.T[1] || b3 >= g.T[2]) continue;   // ragged brick: never referenced
-        const double *src = vin + ((size_t)(4 * b1 + (col >> 2)) * g.N[1] + 4 * b2 + (col & 3)) * g.N[2] + 4 * b3;
+    const double *vin = P.grid[level];
+    // ---- stage the brick: one row of 4 points (x NCOMP) per thread and trip; t3 fastest for coalescing ----
+    for (int r = threadIdx.x; r < BRICK_TILES * 16; r += NWARP * 32) {
+        const int t3 = r % BR3, j = (r / BR3) & 3, t2 = (r / (BR3 * 4)) % BR2, x = r / (BR3 * 4 * BR2);
+        const int b1 = k1, b2 = BR2 * k2 + t2, b3 = BR3 * k3 + t3;
+        if (b2 >= g.T[1] || b3 >= g.T[2]) continue;   // ragged brick: never referenced
+        const double *src = vin + ((size_t)(4 * b1 + x) * g.N[1] + 4 * b2 + j) * g.N[2] + 4 * b3;
         double raw[NCOMP][4];
 #pragma unroll
         for (int k = 0; k < NCOMP; k++) {
@@ -130,7 +118,7 @@ __global__ void __launch_bounds__(NWARP * 32) k_integrate(const __grid_constant_
             const double2 x0 = __ldg(p2), x1 = __ldg(p2 + 1);
             raw[k][0] = x0.x; raw[k][1] = x0.y; raw[k][2] = x1.x; raw[k][3] = x1.y;
         }
-        double *dst = vs + (size_t)lt * (NCOMP * 64) + col * 2;
+        double *dst = vs + ((t2 * BR3 + t3) * 4 + x) * CHS + j * 4;
         if constexpr (DERIV) {
             // w'_i = sum_c Hinv[i][c] w_c, so that w . grad_r f = w' . grad_u f
             double tr[4][4];
@@ -144,54 +132,73 @@ __global__ void __launch_bounds__(NWARP * 32) k_integrate(const __grid_constant_
             }
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                *reinterpret_cast<double2 *>(dst + k * 64) = make_double2(tr[k][0], tr[k][1]);
-                *reinterpret_cast<double2 *>(dst + k * 64 + 32) = make_double2(tr[k][2], tr[k][3]);
+                *reinterpret_cast<double2 *>(dst + k * 16) = make_double2(tr[k][0], tr[k][1]);
+                *reinterpret_cast<double2 *>(dst + k * 16 + 2) = make_double2(tr[k][2], tr[k][3]);
             }
         } else {
             *reinterpret_cast<double2 *>(dst) = make_double2(raw[0][0], raw[0][1]);
-            *reinterpret_cast<double2 *>(dst + 32) = make_double2(raw[0][2], raw[0][3]);
+            *reinterpret_cast<double2 *>(dst + 2) = make_double2(raw[0][2], raw[0][3]);
         }
     }
     __syncthreads();
 
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane >> 2;
     BrickCtx c;
-    c.tasks = tasks;
-    c.entries = entries + P.brick_base[it.level][it.brick];
     c.vs = vs;
-#pragma unroll
-    for (int x = 0; x < 6; x++) c.gm[x] = g.Gm[x];
-    c.o1 = 4 * BRICK * k1; c.o2 = 4 * BRICK * k2; c.o3 = 4 * BRICK * k3;
+    c.gm = g.Gm;
+    c.o1 = 4 * BR1 * k1; c.o2 = 4 * BR2 * k2; c.o3 = 4 * BR3 * k3;
     c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    c.x = lane & 3;
+    const BEntry *ent = entries + ebase;
 
-    unsigned e = it.lo + warp;
-    if (e >= it.hi) return;
-    BEntry en = c.entries[e];
-    PairRec pr = load_pair(tasks, en.task);
-    for (;;) {
-        const unsigned e2 = e + NWARP;
-        const bool more = e2 < it.hi;
-        BEntry en2 = en;
-        PairRec pr2 = pr;
-        if (more) { en2 = c.entries[e2]; pr2 = load_pair(tasks, en2.task); }   // in flight during this entry
-        switch (en.L) {
-            case 0: integ_entry<0, DERIV>(c, en, pr, lane, mom); break;
-            case 1: integ_entry<1, DERIV>(c, en, pr, lane, mom); break;
-            case 2: integ_entry<2, DERIV>(c, en, pr, lane, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV>(c, en, pr, lane, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV>(c, en, pr, lane, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV>(c, en, pr, lane, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV>(c, en, pr, lane, mom); break;
+    // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
+    // warp-uniform); the chunks are dealt to the CTA's warps round robin.
+    int L = -1, cc = 0;
+    unsigned base = 0, hi = 0;
+    auto next_chunk = [&]() -> bool {
+        for (;;) {
+            base += NGRP;
+            if (L < 0 || base >= hi) {
+                do {
+                    L++;
+                    if (L > LMAX) return false;
+                    base = max(it_lo, s_seg[L]);
+                    hi = min(it_hi, s_seg[L + 1]);
+                } while (base >= hi);
+            }
+            if ((cc++ % NWARP) == warp) return true;
         }
-        if (!more) break;
-        en = en2; pr = pr2; e = e2;
+    };
+    bool have = next_chunk();
+    if (!have) return;
+    BEntry en;
+    PairRec pr;
+    en.mask = 0; en.task = 0; en.s[0] = en.s[1] = en.s[2] = 0; en.L = 0; en.pad = 0;
+    pr = PairRec{0, 0, 0, 0, 0, 0, 0, 0};
+    if (base + grp < hi) { en = ent[base + grp]; pr = load_pair(tasks, en.task); }
+    while (have) {
+        const int Lc = L;
+        const bool valid = base + grp < hi;
+        const BEntry enc = en;
+        const PairRec prc = pr;
+        have = next_chunk();
+        if (have && base + grp < hi) { en = ent[base + grp]; pr = load_pair(tasks, en.task); }   // in flight during this chunk
+        switch (Lc) {
+            case 0: integ_entry<0, DERIV>(c, enc, prc, valid, mom); break;
+            case 1: integ_entry<1, DERIV>(c, enc, prc, valid, mom); break;
+            case 2: integ_entry<2, DERIV>(c, enc, prc, valid, mom); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV>(c, enc, prc, valid, mom); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV>(c, enc, prc, valid, mom); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV>(c, enc, prc, valid, mom); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV>(c, enc, prc, valid, mom); break;
+        }
     }
 }
 
 template <int DERIV, int LMAX>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    double *mom, cudaStream_t st) {
-    constexpr int smem = BRICK_TILES * (DERIV ? 4 : 1) * 64 * (int)sizeof(double);
+    constexpr int smem = BRICK_TILES * 4 * chunk_doubles(DERIV ? 4 : 1) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
         const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);

@@ -198,7 +198,8 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
             g.ecut = e;
             g.ntile = g.T[0] * g.T[1] * g.T[2];
-            for (int i = 0; i < 3; i++) g.B[i] = (g.T[i] + BRICK - 1) / BRICK;
+            const int BR[3] = {BR1, BR2, BR3};
+            for (int i = 0; i < 3; i++) g.B[i] = (g.T[i] + BR[i] - 1) / BR[i];
             g.nbrick = g.B[0] * g.B[1] * g.B[2];
             g.dV = hp->omega / ((double)g.N[0] * g.N[1] * g.N[2]);
             for (int c = 0; c < 3; c++)
@@ -414,8 +415,8 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                             rv.push_back(v);
                             // the same visit in the brick lists of the integration kernel
                             const long long bkey = lev_brick0[t.level] +
-                                ((long long)(w1 / BRICK) * g.B[1] + (w2 / BRICK)) * g.B[2] + (w3 / BRICK);
-                            const unsigned bit = 1u << (((w1 % BRICK) * BRICK + (w2 % BRICK)) * BRICK + (w3 % BRICK));
+                                ((long long)(w1 / BR1) * g.B[1] + (w2 / BR2)) * g.B[2] + (w3 / BR3);
+                            const unsigned bit = 1u << ((w2 % BR2) * BR3 + (w3 % BR3));
                             size_t e = rb0;
                             for (; e < rb.size(); e++)
                                 if (rb[e].key == bkey && rb[e].s[0] == v.s[0] && rb[e].s[1] == v.s[1] && rb[e].s[2] == v.s[2]) break;
@@ -489,19 +490,38 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 std::vector<RawEntry>().swap(rb);
             }
             hp->brick_base.resize(nlevel);
+            for (int a = 0; a < nlevel; a++)
+                hp->brick_base[a].assign(bcnt.begin() + lev_brick0[a], bcnt.begin() + lev_brick0[a] + hp->lev[a].nbrick + 1);
+            // inside a brick: by L (the kernel's code path), then by decreasing number of visited blocks so
+            // that the eight lane groups of a warp, which take consecutive entries, finish together
+            parallel_chunks(nbrick_all, 64, nthread, [&](long, long lo, long hi, int) {
+                for (long b = lo; b < hi; b++)
+                    std::stable_sort(hp->bentry.begin() + bcnt[b], hp->bentry.begin() + bcnt[b + 1],
+                                     [](const BEntry &x, const BEntry &y) {
+                                         if (x.L != y.L) return x.L < y.L;
+                                         return __builtin_popcount(x.mask) > __builtin_popcount(y.mask);
+                                     });
+            });
             const unsigned BITEM_MAX = 768;
             std::vector<std::pair<long long, BItem>> tmp;
             for (int a = 0; a < nlevel; a++) {
                 const int nb = hp->lev[a].nbrick;
-                hp->brick_base[a].assign(bcnt.begin() + lev_brick0[a], bcnt.begin() + lev_brick0[a] + nb + 1);
                 for (int b = 0; b < nb; b++) {
                     const long long base = hp->brick_base[a][b];
                     const unsigned n = (unsigned)(hp->brick_base[a][b + 1] - base);
                     if (!n) continue;
+                    BItem proto;
+                    std::memset(&proto, 0, sizeof(proto));
+                    proto.level = a; proto.brick = b; proto.base = base;
+                    {
+                        unsigned cntL[8] = {0};
+                        for (unsigned e = 0; e < n; e++) cntL[hp->bentry[(size_t)(base + e)].L]++;
+                        unsigned acc = 0;
+                        for (int L = 0; L < 8; L++) { proto.seg[L] = acc; acc += cntL[L]; }
+                    }
                     const unsigned nparts = (n + BITEM_MAX - 1) / BITEM_MAX;
                     for (unsigned p = 0; p < nparts; p++) {
-                        BItem it;
-                        it.level = a; it.brick = b;
+                        BItem it = proto;
                         it.lo = (unsigned)((unsigned long long)n * p / nparts);
                         it.hi = (unsigned)((unsigned long long)n * (p + 1) / nparts);
                         long long work = 0;
