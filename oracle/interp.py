@@ -11,7 +11,10 @@ Fourier coefficients of a grid function f are
 
 Eq. (8):  rho~_alpha(G) = F(rho_alpha)(G) if |G| < G_alpha, else 0, with the cutoff
 G_alpha = min_i pi N_alpha,i |b_i| (the sphere inscribed in the level's FFT box) and, in addition, every
-Nyquist plane |m_i| = N_alpha,i / 2 dropped (for a cubic cell the sphere already excludes them).
+Nyquist plane |m_i| = N_alpha,i / 2 dropped (for a cubic cell the sphere already excludes them).  A plane
+wave that sits ON the sphere up to rounding (|G|^2 within 1e-12 relative of G_alpha^2; e.g. m = (12,16,0)
+on a cubic 40^3 level) counts as |G| >= G_alpha, so that the decision does not depend on the order of the
+floating-point operations (TIE below).
 Eq. (7):  rho~(G) = sum_alpha rho~_alpha(G), evaluated on the finest mesh:
     interp_up:      rho_fine(r_n) = sum_G rho~(G) exp(+i G . r_n)
 The paper transforms v back "for each of the multiple grids":
@@ -27,6 +30,9 @@ from __future__ import annotations
 from typing import List, Sequence
 
 import numpy as np
+
+
+TIE = 1e-12   # relative width, in |G|^2, of "on the cutoff sphere"
 
 
 def _bvec(cell) -> np.ndarray:
@@ -54,7 +60,7 @@ def keep_mask(cell, mesh) -> np.ndarray:
     G = 2.0 * np.pi * (m1[..., None] * binv[:, 0] + m2[..., None] * binv[:, 1] + m3[..., None] * binv[:, 2])
     g2 = (G * G).sum(-1)
     gc = g_cut(cell, mesh)
-    ok = g2 < gc * gc
+    ok = g2 < gc * gc * (1.0 - TIE)
     for mi, n in ((m1, N[0]), (m2, N[1]), (m3, N[2])):
         ok &= (2 * np.abs(mi) < n)
     return ok
@@ -112,7 +118,7 @@ def _kept_waves(cell, mesh):
                 if 2 * abs(m1) >= N[0] or 2 * abs(m2) >= N[1] or 2 * abs(m3) >= N[2]:
                     continue
                 G = 2.0 * np.pi * (m1 * binv[:, 0] + m2 * binv[:, 1] + m3 * binv[:, 2])
-                if float(G @ G) < gc * gc:
+                if float(G @ G) < gc * gc * (1.0 - TIE):
                     out.append(((m1, m2, m3), G))
     return out
 

@@ -3,7 +3,7 @@
     python -m paper_2603_24881_b200.build [--force]
 
 The library holds the host plan builder (csrc/plan.cpp) and the CUDA kernels plus the C ABI
-(csrc/gpw_cuda.cu); include/gpw.h is the interface.  nvcc cross-compiles without a GPU.
+(csrc/gpw_api.cu, collocate.cu, integrate.cu, interp.cu); include/gpw.h is the interface.  nvcc cross-compiles without a GPU.
 """
 from __future__ import annotations
 
@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpw.so")
-SOURCES = ["plan.cpp", "gpw_api.cu", "collocate.cu", "integrate.cu"]
+SOURCES = ["plan.cpp", "gpw_api.cu", "collocate.cu", "integrate.cu", "interp.cu"]
 HEADERS = ["gpw_internal.h", "gpw_math.cuh", "gpw_kernels.cuh"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

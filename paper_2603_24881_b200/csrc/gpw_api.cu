@@ -91,6 +91,7 @@ struct gpw_plan {
     bool timing = false;
     cudaEvent_t ev[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
     bool ev_valid[2] = {false, false};
+    InterpState *interp = nullptr;   // cuFFT plans and scratch of gpw_interp_up / gpw_restrict_down (first use)
 };
 
 namespace {
@@ -112,6 +113,8 @@ bool upload(T **dst, const T *src, size_t n, long &bytes, const char *what) {
 }
 
 void free_device(gpw_plan *p) {
+    interp_free(p->interp);
+    p->interp = nullptr;
     for (int w = 0; w < 2; w++)
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
@@ -216,7 +219,7 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
     out->nitem = (long)hp->item.size();
     out->ncoef_total = (long)hp->ncoef_total;
     out->build_seconds = hp->build_seconds;
-    out->device_bytes = p->device_bytes;
+    out->device_bytes = p->device_bytes + interp_bytes(p->interp);
     return GPW_OK;
 }
 
@@ -345,13 +348,22 @@ int gpw_dfma_peak(double min_seconds, double *tflops_out, int *sm_count_out) {
     return GPW_OK;
 }
 
-int gpw_interp_up(gpw_plan *, const double *const *, int, double *, void *) {
-    set_error("gpw_interp_up: not built yet");
-    return GPW_EUNSUPPORTED;
+int gpw_interp_up(gpw_plan *p, const double *const *rho_dev, int ncomp, double *rho_fine_dev, void *cuda_stream) {
+    if (!p || !rho_dev || !rho_fine_dev) { set_error("gpw_interp_up: null argument"); return GPW_EINVAL; }
+    if (ncomp < 1) { set_error("gpw_interp_up: ncomp must be >= 1"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_interp_up: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    for (int a = 0; a < p->hp->nlevel; a++)
+        if (!rho_dev[a]) { set_error("gpw_interp_up: null level pointer"); return GPW_EINVAL; }
+    return interp_up(p->hp, &p->interp, rho_dev, ncomp, rho_fine_dev, (cudaStream_t)cuda_stream);
 }
-int gpw_restrict_down(gpw_plan *, const double *, int, double *const *, void *) {
-    set_error("gpw_restrict_down: not built yet");
-    return GPW_EUNSUPPORTED;
+
+int gpw_restrict_down(gpw_plan *p, const double *v_fine_dev, int ncomp, double *const *v_dev, void *cuda_stream) {
+    if (!p || !v_fine_dev || !v_dev) { set_error("gpw_restrict_down: null argument"); return GPW_EINVAL; }
+    if (ncomp < 1) { set_error("gpw_restrict_down: ncomp must be >= 1"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_restrict_down: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    for (int a = 0; a < p->hp->nlevel; a++)
+        if (!v_dev[a]) { set_error("gpw_restrict_down: null level pointer"); return GPW_EINVAL; }
+    return interp_down(p->hp, &p->interp, v_fine_dev, ncomp, v_dev, (cudaStream_t)cuda_stream);
 }
 
 }  // extern "C"

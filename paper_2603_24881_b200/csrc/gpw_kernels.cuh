@@ -37,4 +37,11 @@ cudaError_t launch_collocate(const GridParams &P, const TaskK *tasks, const Visi
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
                              int nitem, double *mom, int deriv, int max_L, cudaStream_t st);
 
+// interp.cu: Eq. (7)-(8) with cuFFT; the state (plans, scratch) is created on first use; return a gpw_status
+struct InterpState;
+int interp_up(const HostPlan *hp, InterpState **st, const double *const *rho, int ncomp, double *fine, cudaStream_t s);
+int interp_down(const HostPlan *hp, InterpState **st, const double *fine, int ncomp, double *const *v, cudaStream_t s);
+void interp_free(InterpState *st);
+long interp_bytes(const InterpState *st);
+
 }  // namespace gpw

@@ -99,6 +99,10 @@ def test_eval_without_device_fails_loudly():
     assert b"no CPU path" in lib.gpw_last_error()
     rc = lib.gpw_eval_mat(plan._h, dummy, 0, ctypes.c_void_p(8), None)
     assert rc == binding.GPW_ECUDA
+    rc = lib.gpw_interp_up(plan._h, dummy, 1, ctypes.c_void_p(8), None)
+    assert rc == binding.GPW_ECUDA and b"no CPU path" in lib.gpw_last_error()
+    rc = lib.gpw_restrict_down(plan._h, ctypes.c_void_p(8), 1, dummy, None)
+    assert rc == binding.GPW_ECUDA and b"no CPU path" in lib.gpw_last_error()
 
 
 def test_model_flops_convention():

@@ -147,3 +147,15 @@ def test_band_limited_fine_field_is_its_own_image():
     f = np.fft.ifftn(spec).real
     assert np.abs(interp.interp_up(TRICLINIC, meshes, [f]) - f).max() <= 1e-14
     assert np.abs(interp.restrict_down(TRICLINIC, meshes, f)[0] - f).max() <= 1e-14
+
+
+def test_wave_on_the_cutoff_sphere_is_dropped_whatever_the_rounding():
+    # cubic 40^3 level: m = (12,16,0) has |m|^2 = 400 = (N/2)^2 exactly -> |G| = G_alpha -> dropped; for
+    # several edge lengths (different roundings of 2 pi m / L) the decision must be the same
+    for L in (7.0, 7.3, 9.123456789, 37.2):
+        keep = interp.keep_mask(np.diag([L, L, L]), [40, 40, 40])
+        assert not keep[12, 16, 0] and not keep[16, 12, 0] and not keep[0, -12, 16]
+        assert keep[12, 15, 0] and keep[11, 16, 3]
+        m = np.arange(-19, 20)
+        want = sum(1 for a in m for b in m for c in m if a * a + b * b + c * c < 400)
+        assert int(keep.sum()) == want
