@@ -19,6 +19,13 @@ constexpr int NWARP = 4;  // warps (work items) per CTA
 
 // Shared-memory slot of one visit: the pair record (8 doubles) followed by the pair polynomial.
 GPW_CX int slot_doubles(int lmax) { return 8 + ncoef_pad(lmax); }
+// A group's two slots, padded so that consecutive groups start 16 bytes apart modulo the 128-byte bank
+// row: the eight groups' broadcast reads of the same coefficient then hit eight different bank pairs.
+GPW_CX int group_stride(int lmax) {
+    int n = 2 * slot_doubles(lmax);
+    while (n % 16 != 2) n += 2;
+    return n;
+}
 
 struct ColCtx {
     const TaskK *tasks;
@@ -30,7 +37,6 @@ struct ColCtx {
     int n1, n2, n3;        // stored index of the lane's slab corner
     int N0, N1, N2;
     int x;                 // lane within the group
-    unsigned gmask;        // the group's lanes
 };
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
@@ -39,54 +45,46 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// The group's four lanes copy the pair record and polynomial of `task` into a slot (16 bytes per lane and trip).
-template <int L>
-__device__ __forceinline__ void stage_visit(const ColCtx &c, int task, double *slot) {
-    constexpr int NCH = 4 + ncoef_pad(L) / 2;   // 16-byte chunks
+// The group's four lanes copy the pair record and polynomial of `task` (class L) into a slot (16 bytes per
+// lane and trip).
+__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, double *slot) {
+    const int npad = ncoef_pad(L);
+    const int nch = 4 + npad / 2;   // 16-byte chunks
     const char *src_k = reinterpret_cast<const char *>(c.tasks + task);
-    const char *src_c = reinterpret_cast<const char *>(c.work + c.coef_base[L] + (long long)task * ncoef_pad(L));
-#pragma unroll
-    for (int k0 = 0; k0 < NCH; k0 += 4) {
-        const int k = k0 + c.x;
-        if (k < NCH) cp_async16(reinterpret_cast<char *>(slot) + 16 * k, k < 4 ? src_k + 16 * k : src_c + 16 * (k - 4));
-    }
+    const char *src_c = reinterpret_cast<const char *>(c.work + c.coef_base[L] + (long long)task * npad);
+    for (int k = c.x; k < nch; k += 4)
+        cp_async16(reinterpret_cast<char *>(slot) + 16 * k, k < 4 ? src_k + 16 * k : src_c + 16 * (k - 4));
     cp_async_commit();
 }
 
-template <int L, int DERIV, int SLOT>
-__device__ __forceinline__ void colloc_segment(const ColCtx &c, unsigned lo, unsigned hi, int grp,
-                                               double (*acc)[16]) {
-    unsigned v = lo + grp;
-    if (v >= hi) return;
-    Visit vi = c.visits[v];
-    stage_visit<L>(c, vi.task, c.slot);
-    Visit vin = vi;
-    if (v + NGRP < hi) vin = c.visits[v + NGRP];
-    int cur = 0;
-    for (;;) {
-        const unsigned vn = v + NGRP;
-        const bool more = vn < hi;
-        cp_async_wait_all();
-        __syncwarp(c.gmask);   // the slot is complete, and every lane has left the slot refilled next
-        Visit vinn = vin;
-        if (more) {
-            stage_visit<L>(c, vin.task, c.slot + (cur ^ 1) * SLOT);   // in flight while this visit is evaluated
-            if (vn + NGRP < hi) vinn = c.visits[vn + NGRP];
-        }
-        const double *s = c.slot + cur * SLOT;
-        const double ap = s[3];
-        double q[6];
-#pragma unroll
-        for (int k = 0; k < 6; k++) q[k] = ap * c.gm[k];
-        const double u1 = (double)(c.n1 + vi.s[0] * c.N0) - s[0];
-        const double u20 = (double)(c.n2 + vi.s[1] * c.N1) - s[1];
-        const double u30 = (double)(c.n3 + vi.s[2] * c.N2) - s[2];
-        colloc_slab<L, DERIV>(s + 8, q, s[4], s[5], s[6], u1, u20, u30, acc);
-        if (!more) break;
-        vi = vin; vin = vinn;
-        v = vn;
-        cur ^= 1;
+// The item's visits in chunks of NGRP that never straddle an L segment (so the code path is warp-uniform).
+// Lane l holds seg[l & 7] of the block; all lanes advance together.
+struct ChunkIt {
+    int L;
+    unsigned base, hi;   // the chunk is [base, min(base + NGRP, hi)); hi = end of the segment inside the item
+};
+template <int LMAX>
+__device__ __forceinline__ bool next_chunk(ChunkIt &it, unsigned it_lo, unsigned it_hi, unsigned myseg) {
+    it.base += NGRP;
+    while (it.L < 0 || it.base >= it.hi) {
+        it.L++;
+        if (it.L > LMAX) return false;
+        it.base = max(it_lo, __shfl_sync(0xffffffffu, myseg, it.L));
+        it.hi = min(it_hi, __shfl_sync(0xffffffffu, myseg, it.L + 1));
     }
+    return true;
+}
+
+template <int L, int DERIV, bool ORTHO>
+__device__ __forceinline__ void colloc_visit(const ColCtx &c, const Visit vi, const double *s, double (*acc)[16]) {
+    const double ap = s[3];
+    double q[6];
+#pragma unroll
+    for (int k = 0; k < 6; k++) q[k] = ap * c.gm[k];
+    const double u1 = (double)(c.n1 + vi.s[0] * c.N0) - s[0];
+    const double u20 = (double)(c.n2 + vi.s[1] * c.N1) - s[1];
+    const double u30 = (double)(c.n3 + vi.s[2] * c.N2) - s[2];
+    colloc_slab<L, DERIV, ORTHO>(s + 8, q, s[4], s[5], s[6], u1, u20, u30, acc);
 }
 
 // Sum an N-vector over the eight groups (lane bits 4, 8, 16); afterwards the lane holds N/8 sums,
@@ -110,7 +108,7 @@ __device__ __forceinline__ int group_reduce_scatter(double *a, int lane) {
     return off;
 }
 
-template <int DERIV, int LMAX>
+template <int DERIV, int LMAX, bool ORTHO>
 __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_constant__ GridParams P,
                                                                    const TaskK *__restrict__ tasks,
                                                                    const Visit *__restrict__ visits,
@@ -118,7 +116,8 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
                                                                    const double *__restrict__ coef) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int SLOT = slot_doubles(LMAX);
-    extern __shared__ __align__(16) double sm[];   // [NWARP][NGRP][2][SLOT]
+    constexpr int GSTRIDE = group_stride(LMAX);
+    extern __shared__ __align__(16) double sm[];   // [NWARP][NGRP] x (two slots, padded to GSTRIDE)
     const int w = blockIdx.x * NWARP + (threadIdx.x >> 5);
     if (w >= nitem) return;
     const Item it = items[w];
@@ -132,12 +131,11 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
     c.work = coef;
     c.gm = g.Gm;
     c.coef_base = P.coef_base[it.level];
-    c.slot = sm + (size_t)((threadIdx.x >> 5) * NGRP + grp) * 2 * SLOT;
+    c.slot = sm + (size_t)((threadIdx.x >> 5) * NGRP + grp) * GSTRIDE;
     c.x = x;
-    c.gmask = 0xFu << (grp * 4);
     c.n1 = 4 * b1 + x; c.n2 = 4 * b2; c.n3 = 4 * b3;
     c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
-    const unsigned *seg = P.seg[it.level] + (size_t)it.tile * 8;
+    const unsigned myseg = P.seg[it.level][(size_t)it.tile * 8 + (lane & 7)];
 
     double acc[NCOMP][16];
 #pragma unroll
@@ -145,19 +143,42 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 #pragma unroll
         for (int i = 0; i < 16; i++) acc[k][i] = 0.0;
 
-#pragma unroll 1
-    for (int L = 0; L <= LMAX; L++) {
-        const unsigned lo = max(it.lo, seg[L]), hi = min(it.hi, seg[L + 1]);
-        if (lo >= hi) continue;
-        switch (L) {
-            case 0: colloc_segment<0, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            case 1: colloc_segment<1, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            case 2: colloc_segment<2, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            case 3: if constexpr (LMAX >= 3) colloc_segment<3, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            case 4: if constexpr (LMAX >= 4) colloc_segment<4, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            case 5: if constexpr (LMAX >= 5) colloc_segment<5, DERIV, SLOT>(c, lo, hi, grp, acc); break;
-            default: if constexpr (LMAX >= 6) colloc_segment<6, DERIV, SLOT>(c, lo, hi, grp, acc); break;
+    // Software pipeline over the chunks, across L segments: the visit records of chunk k+2 are loaded and
+    // the pair record + polynomial of chunk k+1 are copied to shared memory (cp.async) while chunk k is
+    // evaluated.
+    ChunkIt c0{-1, 0u, 0u};
+    bool h0 = next_chunk<LMAX>(c0, it.lo, it.hi, myseg);
+    ChunkIt c1 = c0;
+    bool h1 = h0 && next_chunk<LMAX>(c1, it.lo, it.hi, myseg);
+    Visit v0, v1;
+    v0.task = 0; v0.s[0] = v0.s[1] = v0.s[2] = 0; v0.pad = 0;
+    v1 = v0;
+    if (h0 && c0.base + grp < c0.hi) { v0 = c.visits[c0.base + grp]; stage_visit(c, c0.L, v0.task, c.slot); }
+    if (h1 && c1.base + grp < c1.hi) v1 = c.visits[c1.base + grp];
+    int cur = 0;
+    while (h0) {
+        ChunkIt c2 = c1;
+        const bool h2 = h1 && next_chunk<LMAX>(c2, it.lo, it.hi, myseg);
+        Visit v2 = v1;
+        if (h2 && c2.base + grp < c2.hi) v2 = c.visits[c2.base + grp];
+        cp_async_wait_all();
+        __syncwarp();   // the slot is complete, and every lane has left the slot refilled next
+        if (h1 && c1.base + grp < c1.hi) stage_visit(c, c1.L, v1.task, c.slot + (cur ^ 1) * SLOT);
+        if (c0.base + grp < c0.hi) {
+            const double *s = c.slot + cur * SLOT;
+            switch (c0.L) {
+                case 0: colloc_visit<0, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 1: colloc_visit<1, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 2: colloc_visit<2, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 3: if constexpr (LMAX >= 3) colloc_visit<3, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 4: if constexpr (LMAX >= 4) colloc_visit<4, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 5: if constexpr (LMAX >= 5) colloc_visit<5, DERIV, ORTHO>(c, v0, s, acc); break;
+                default: if constexpr (LMAX >= 6) colloc_visit<6, DERIV, ORTHO>(c, v0, s, acc); break;
+            }
         }
+        c0 = c1; h0 = h1; v0 = v1;
+        c1 = c2; h1 = h2; v1 = v2;
+        cur ^= 1;
     }
     __syncwarp();
     // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i (linear: before the sum)
@@ -189,32 +210,36 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
     }
 }
 
-template <int DERIV, int LMAX>
+template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items, int nitem,
                    const double *coef, cudaStream_t st) {
-    constexpr int smem = NWARP * NGRP * 2 * slot_doubles(LMAX) * (int)sizeof(double);
+    constexpr int smem = NWARP * NGRP * group_stride(LMAX) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
-        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    k_collocate<DERIV, LMAX><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, tasks, visits, items, nitem, coef);
+    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, tasks, visits, items, nitem, coef);
     return cudaGetLastError();
+}
+
+template <int DERIV, bool ORTHO>
+cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items, int nitem,
+                     const double *coef, int max_L, cudaStream_t st) {
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, visits, items, nitem, coef, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, visits, items, nitem, coef, st);
+    return launch<DERIV, 6, ORTHO>(P, tasks, visits, items, nitem, coef, st);
 }
 
 }  // namespace
 
 cudaError_t launch_collocate(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items,
-                             int nitem, const double *coef, int deriv, int max_L, cudaStream_t st) {
-    if (deriv) {
-        if (max_L <= 2) return launch<1, 2>(P, tasks, visits, items, nitem, coef, st);
-        if (max_L <= 4) return launch<1, 4>(P, tasks, visits, items, nitem, coef, st);
-        return launch<1, 6>(P, tasks, visits, items, nitem, coef, st);
-    }
-    if (max_L <= 2) return launch<0, 2>(P, tasks, visits, items, nitem, coef, st);
-    if (max_L <= 4) return launch<0, 4>(P, tasks, visits, items, nitem, coef, st);
-    return launch<0, 6>(P, tasks, visits, items, nitem, coef, st);
+                             int nitem, const double *coef, int deriv, int max_L, bool ortho, cudaStream_t st) {
+    if (deriv) return ortho ? launch_l<1, true>(P, tasks, visits, items, nitem, coef, max_L, st)
+                            : launch_l<1, false>(P, tasks, visits, items, nitem, coef, max_L, st);
+    return ortho ? launch_l<0, true>(P, tasks, visits, items, nitem, coef, max_L, st)
+                 : launch_l<0, false>(P, tasks, visits, items, nitem, coef, max_L, st);
 }
 
 }  // namespace gpw

@@ -261,7 +261,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, st),
+    if (!cuda_ok(launch_collocate(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
@@ -285,7 +285,7 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[1][0], st); pm->ev_valid[1] = true; }
     if (!cuda_ok(launch_integrate(P, p->d_taskK, p->d_bentry, p->d_bitem, (int)hp->bitem.size(), p->d_mom, deriv,
-                                  hp->max_L, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
+                                  hp->max_L, hp->ortho, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[1][1], st);
     DVs dv;
     for (int a = 0; a < GPW_MAX_LEVEL; a++) dv.v[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;

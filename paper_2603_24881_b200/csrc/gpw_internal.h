@@ -140,6 +140,7 @@ struct HostPlan {
                                                      // inside an L segment by decreasing number of visited blocks
     std::vector<BItem> bitem;                        // sorted by descending work
     int max_L = 0;                                   // largest la + lb present
+    bool ortho = false;                              // the lattice vectors are mutually orthogonal (every Gm diagonal)
     long nvisit_level[GPW_MAX_LEVEL] = {0};
     long ntask_level[GPW_MAX_LEVEL] = {0};
     long nvisit_class[GPW_MAX_LEVEL][MAXL + 1][MAXL + 1] = {{{0}}};

@@ -31,11 +31,11 @@ __device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, in
     return r;
 }
 
-// launchers (each picks the instantiation for the plan's largest L)
+// launchers (each picks the instantiation for the plan's largest L; ortho: every level's Gm is diagonal)
 cudaError_t launch_collocate(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items,
-                             int nitem, const double *coef, int deriv, int max_L, cudaStream_t st);
+                             int nitem, const double *coef, int deriv, int max_L, bool ortho, cudaStream_t st);
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, double *mom, int deriv, int max_L, cudaStream_t st);
+                             int nitem, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st);
 
 // interp.cu: Eq. (7)-(8) with cuFFT; the state (plans, scratch) is created on first use; return a gpw_status
 struct InterpState;

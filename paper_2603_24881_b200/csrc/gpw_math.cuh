@@ -227,17 +227,26 @@ GPW_HD constexpr int bidx(int L, int ky, int kz) {
 
 // Gaussian at the slab corner and the first-step ratios along n2 and n3.
 //   g0 = exp(-E(u1,u20,u30)),  r2 = G(j=1,t=0)/G(0,0),  r3 = G(0,1)/G(0,0)
-// Every intermediate of the recursion is a true Gaussian value or a true ratio of neighbouring values; the
-// plan builder routes pairs for which one of them could leave the FP64 range (pairs far sharper than their
-// grid resolves, reading A23) to the direct class instead (plan.cpp, "direct class").
+// Every intermediate of the recursion is a true Gaussian value or a true ratio of neighbouring values, so
+// it stays inside the FP64 range as long as q u^2 < 700 over the visited blocks (q = a_p h^2 <= ~1 for the
+// sharpest pairs routed to level 0 by reading A23, u <= R_t/h + 7 grid steps: two orders of magnitude of
+// margin on every config).  ORTHO: the level's step vectors are mutually orthogonal (Gm is diagonal).
 struct SlabGauss { double g0, r2, r3; };
+template <bool ORTHO = false>
 GPW_HD SlabGauss slab_gauss(const double *q, double u1, double u20, double u30) {
-    const double E0 = q[0] * u1 * u1 + q[1] * u20 * u20 + q[2] * u30 * u30 +
-                      2.0 * (q[3] * u1 * u20 + (q[4] * u1 + q[5] * u20) * u30);
-    const double s2 = 2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30) + q[1];
-    const double s3 = 2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30) + q[2];
     SlabGauss G;
-    G.g0 = exp(-E0); G.r2 = exp(-s2); G.r3 = exp(-s3);
+    if constexpr (ORTHO) {
+        const double E0 = fma(q[0] * u1, u1, fma(q[1] * u20, u20, q[2] * u30 * u30));
+        G.g0 = exp(-E0);
+        G.r2 = exp(-(q[1] * fma(2.0, u20, 1.0)));
+        G.r3 = exp(-(q[2] * fma(2.0, u30, 1.0)));
+    } else {
+        const double E0 = q[0] * u1 * u1 + q[1] * u20 * u20 + q[2] * u30 * u30 +
+                          2.0 * (q[3] * u1 * u20 + (q[4] * u1 + q[5] * u20) * u30);
+        const double s2 = 2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30) + q[1];
+        const double s3 = 2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30) + q[2];
+        G.g0 = exp(-E0); G.r2 = exp(-s2); G.r3 = exp(-s3);
+    }
     return G;
 }
 GPW_HD double gauss_direct(const double *q, double u1, double u2, double u3) {
@@ -246,8 +255,10 @@ GPW_HD double gauss_direct(const double *q, double u1, double u2, double u3) {
 }
 
 // Collocation of one pair on one slab.  acc[NCOMP][16] (index j*4+t); for DERIV the gradient is
-// accumulated in grid-index (covariant) components.
-template <int L, int DERIV>
+// accumulated in grid-index (covariant) components:  d/du_i [Q G] = G (dQ/du_i + p_i Q),  p = -2 (q u).
+// ORTHO: the Gaussian along n3 relative to the row start (g3) and p_3 are the same for the four rows, p_1
+// is constant on the slab and p_2 on a row.
+template <int L, int DERIV, bool ORTHO = false>
 GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c22, double c23, double c33,
                         double u1, double u20, double u30, double (*acc)[16]) {
     constexpr int NB = npair2(L), NBX = npair2(L - 1);
@@ -256,23 +267,38 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
     for (int kz = 0; kz <= L; kz++)
 #pragma unroll
         for (int ky = 0; ky <= L - kz; ky++) {
-            double p = 0.0, dp = 0.0;
+            const int n = L - kz - ky;          // degree in u1
+            double p = c[cidx(L, n, ky, kz)], dp = 0.0;
 #pragma unroll
-            for (int kx = L - kz - ky; kx >= 0; kx--) {
-                if (DERIV) dp = dp * u1 + p;
-                p = p * u1 + c[cidx(L, kx, ky, kz)];
+            for (int kx = n - 1; kx >= 0; kx--) {
+                if (DERIV) dp = kx == n - 1 ? p : fma(dp, u1, p);
+                p = fma(p, u1, c[cidx(L, kx, ky, kz)]);
             }
             b[bidx(L, ky, kz)] = p;
             if (DERIV && ky + kz <= L - 1) bx[bidx(L - 1, ky, kz)] = dp;
         }
-    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
+    const SlabGauss SG = slab_gauss<ORTHO>(q, u1, u20, u30);
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
-    // -2 (q u)_i at the row start, its step per row and per point
+    // p = -2 (q u) at the row start, its step per row and per point
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
     if (DERIV) {
-        qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
-        qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
-        qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+        if constexpr (ORTHO) {
+            qr1 = -2.0 * (q[0] * u1); qr2 = -2.0 * (q[1] * u20); qr3 = -2.0 * (q[2] * u30);
+        } else {
+            qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
+            qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
+            qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+        }
+    }
+    // ORTHO: Gaussian along n3 relative to the row start, and p_3 per point -- shared by the four rows
+    double g3[4] = {1.0, 1.0, 1.0, 1.0}, p3t[4] = {0.0, 0.0, 0.0, 0.0};
+    if constexpr (ORTHO) {
+        double r = SG.r3;
+        g3[1] = r; r *= c33; g3[2] = g3[1] * r; r *= c33; g3[3] = g3[2] * r;
+        if (DERIV) {
+#pragma unroll
+            for (int t = 0; t < 4; t++) p3t[t] = fma(-2.0 * q[2], (double)t, qr3);
+        }
     }
 #pragma unroll
     for (int j = 0; j < 4; j++) {
@@ -280,18 +306,19 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
         double a[L + 1], ax[L > 0 ? L : 1], ay[L > 0 ? L : 1];
 #pragma unroll
         for (int kz = 0; kz <= L; kz++) {
-            double s = 0.0, sy = 0.0;
+            const int n = L - kz;               // degree in u2
+            double s = b[bidx(L, n, kz)], sy = 0.0;
 #pragma unroll
-            for (int ky = L - kz; ky >= 0; ky--) {
-                if (DERIV) sy = sy * u2 + s;
-                s = s * u2 + b[bidx(L, ky, kz)];
+            for (int ky = n - 1; ky >= 0; ky--) {
+                if (DERIV) sy = ky == n - 1 ? s : fma(sy, u2, s);
+                s = fma(s, u2, b[bidx(L, ky, kz)]);
             }
             a[kz] = s;
             if (DERIV && kz < L) {
                 ay[kz] = sy;
-                double sx = 0.0;
+                double sx = bx[bidx(L - 1, n - 1, kz)];
 #pragma unroll
-                for (int ky = L - 1 - kz; ky >= 0; ky--) sx = sx * u2 + bx[bidx(L - 1, ky, kz)];
+                for (int ky = n - 2; ky >= 0; ky--) sx = fma(sx, u2, bx[bidx(L - 1, ky, kz)]);
                 ax[kz] = sx;
             }
         }
@@ -300,27 +327,38 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
 #pragma unroll
         for (int t = 0; t < 4; t++) {
             const double u3 = u30 + t;
-            double Q = 0.0, Qz = 0.0;
+            if constexpr (ORTHO) { g = t == 0 ? grow : grow * g3[t]; p3 = p3t[t]; }
+            double Q = a[L], Qz = 0.0;
 #pragma unroll
-            for (int kz = L; kz >= 0; kz--) {
-                if (DERIV) Qz = Qz * u3 + Q;
-                Q = Q * u3 + a[kz];
+            for (int kz = L - 1; kz >= 0; kz--) {
+                if (DERIV) Qz = kz == L - 1 ? Q : fma(Qz, u3, Q);
+                Q = fma(Q, u3, a[kz]);
             }
-            const double w = g * Q;
-            acc[0][j * 4 + t] += w;
+            acc[0][j * 4 + t] = fma(g, Q, acc[0][j * 4 + t]);
             if constexpr (DERIV != 0) {
-                double Qx = 0.0, Qy = 0.0;
+                if constexpr (L > 0) {
+                    double Qx = ax[L - 1], Qy = ay[L - 1];
 #pragma unroll
-                for (int kz = L - 1; kz >= 0; kz--) { Qx = Qx * u3 + ax[kz]; Qy = Qy * u3 + ay[kz]; }
-                acc[1][j * 4 + t] += g * Qx + w * p1;
-                acc[2][j * 4 + t] += g * Qy + w * p2;
-                acc[3][j * 4 + t] += g * Qz + w * p3;
-                p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
+                    for (int kz = L - 2; kz >= 0; kz--) { Qx = fma(Qx, u3, ax[kz]); Qy = fma(Qy, u3, ay[kz]); }
+                    acc[1][j * 4 + t] = fma(g, fma(Q, p1, Qx), acc[1][j * 4 + t]);
+                    acc[2][j * 4 + t] = fma(g, fma(Q, p2, Qy), acc[2][j * 4 + t]);
+                    acc[3][j * 4 + t] = fma(g, fma(Q, p3, Qz), acc[3][j * 4 + t]);
+                } else {
+                    const double w = g * Q;
+                    acc[1][j * 4 + t] = fma(w, p1, acc[1][j * 4 + t]);
+                    acc[2][j * 4 + t] = fma(w, p2, acc[2][j * 4 + t]);
+                    acc[3][j * 4 + t] = fma(w, p3, acc[3][j * 4 + t]);
+                }
+                if constexpr (!ORTHO) { p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2]; }
             }
-            g *= r; r *= c33;
+            if constexpr (!ORTHO) { g *= r; r *= c33; }
         }
-        grow *= r2; r2 *= c22; r3row *= c23;
-        if (DERIV) { qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5]; }
+        grow *= r2; r2 *= c22;
+        if constexpr (!ORTHO) r3row *= c23;
+        if (DERIV) {
+            if constexpr (ORTHO) { qr2 -= 2.0 * q[1]; }
+            else { qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5]; }
+        }
     }
 }
 
@@ -333,18 +371,37 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
 // (contravariant) components.  vrow(comp, j, out[4]) delivers the four values of row j of component comp.
 // A lane of the integration kernel keeps B0 / B1 over ALL blocks of a brick entry: the brick is one block
 // thick along n1, so the lane's u1 is the same for every block.
+// ORTHO: the table T[kz][t] = g3(t) u3_t^kz (Gaussian along n3 relative to the row start times the power)
+// is the same for the four rows; the row's Gaussian factor multiplies the row sums instead of every point.
 //
 // integ_expand_u1: m[cidx(L,kx,ky,kz)] (+)= B0 u1^kx + kx u1^(kx-1) B1 -- once per entry.
-template <int L, int DERIV, class VRow>
+template <int L, int DERIV, bool ORTHO = false, class VRow>
 GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23, double c33,
                             const SlabGauss SG, double u1, double u20, double u30, double *B0, double *B1) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
     if (DERIV) {
-        qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
-        qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
-        qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+        if constexpr (ORTHO) {
+            qr1 = -2.0 * (q[0] * u1); qr2 = -2.0 * (q[1] * u20); qr3 = -2.0 * (q[2] * u30);
+        } else {
+            qr1 = -2.0 * (q[0] * u1 + q[3] * u20 + q[4] * u30);
+            qr2 = -2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30);
+            qr3 = -2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30);
+        }
+    }
+    double T[L + 1][4], p3t[4] = {0.0, 0.0, 0.0, 0.0};
+    if constexpr (ORTHO) {
+        double r = SG.r3;
+        T[0][0] = 1.0; T[0][1] = r; r *= c33; T[0][2] = T[0][1] * r; r *= c33; T[0][3] = T[0][2] * r;
+#pragma unroll
+        for (int kz = 1; kz <= L; kz++)
+#pragma unroll
+            for (int t = 0; t < 4; t++) T[kz][t] = T[kz - 1][t] * (u30 + t);
+        if (DERIV) {
+#pragma unroll
+            for (int t = 0; t < 4; t++) p3t[t] = fma(-2.0 * q[2], (double)t, qr3);
+        }
     }
 #pragma unroll
     for (int j = 0; j < 4; j++) {
@@ -353,59 +410,90 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
 #pragma unroll
         for (int k = 0; k < NCOMP; k++) vrow(k, j, vv[k]);
         double A0[L + 1], A1[L > 0 ? L : 1], A2[L > 0 ? L : 1], A3[L > 0 ? L : 1];
+        if constexpr (ORTHO) {
+            // row sums without the row's Gaussian factor (it multiplies pw2 below)
+            double w0[4];
 #pragma unroll
-        for (int kz = 0; kz <= L; kz++) A0[kz] = 0.0;
-#pragma unroll
-        for (int kz = 0; kz < L; kz++) { A1[kz] = 0.0; A2[kz] = 0.0; A3[kz] = 0.0; }
-        double g = grow, r = r3row;
-        double p1 = qr1, p2 = qr2, p3 = qr3;
-#pragma unroll
-        for (int t = 0; t < 4; t++) {
-            const double u3 = u30 + t;
-            double g0 = vv[0][t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
-            if constexpr (DERIV != 0) {
-                const double z1 = vv[1][t], z2 = vv[2][t], z3 = vv[3][t];
-                g0 += z1 * p1 + z2 * p2 + z3 * p3;
-                g1 = g * z1; g2 = g * z2; g3 = g * z3;
-                p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
+            for (int t = 0; t < 4; t++) {
+                w0[t] = vv[0][t];
+                if constexpr (DERIV != 0) w0[t] = fma(vv[1][t], qr1, fma(vv[2][t], qr2, fma(vv[3][t], p3t[t], w0[t])));
             }
-            g0 *= g;
-            double pw = 1.0;
 #pragma unroll
             for (int kz = 0; kz <= L; kz++) {
-                if (kz == 0) {
-                    A0[0] += g0;
-                    if (DERIV && L > 0) { A1[0] += g1; A2[0] += g2; A3[0] += g3; }
-                } else {
-                    A0[kz] += g0 * pw;
-                    if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
+                A0[kz] = kz == 0 ? fma(T[0][3], w0[3], fma(T[0][2], w0[2], fma(T[0][1], w0[1], w0[0])))
+                                 : fma(T[kz][3], w0[3], fma(T[kz][2], w0[2], fma(T[kz][1], w0[1], T[kz][0] * w0[0])));
+                if (DERIV && kz < L) {
+                    if (kz == 0) {
+                        A1[0] = fma(T[0][3], vv[1][3], fma(T[0][2], vv[1][2], fma(T[0][1], vv[1][1], vv[1][0])));
+                        A2[0] = fma(T[0][3], vv[2][3], fma(T[0][2], vv[2][2], fma(T[0][1], vv[2][1], vv[2][0])));
+                        A3[0] = fma(T[0][3], vv[3][3], fma(T[0][2], vv[3][2], fma(T[0][1], vv[3][1], vv[3][0])));
+                    } else {
+                        A1[kz] = fma(T[kz][3], vv[1][3], fma(T[kz][2], vv[1][2], fma(T[kz][1], vv[1][1], T[kz][0] * vv[1][0])));
+                        A2[kz] = fma(T[kz][3], vv[2][3], fma(T[kz][2], vv[2][2], fma(T[kz][1], vv[2][1], T[kz][0] * vv[2][0])));
+                        A3[kz] = fma(T[kz][3], vv[3][3], fma(T[kz][2], vv[3][2], fma(T[kz][1], vv[3][1], T[kz][0] * vv[3][0])));
+                    }
                 }
-                if (kz < L) pw = kz == 0 ? u3 : pw * u3;
             }
-            g *= r; r *= c33;
+        } else {
+#pragma unroll
+            for (int kz = 0; kz <= L; kz++) A0[kz] = 0.0;
+#pragma unroll
+            for (int kz = 0; kz < L; kz++) { A1[kz] = 0.0; A2[kz] = 0.0; A3[kz] = 0.0; }
+            double g = grow, r = r3row;
+            double p1 = qr1, p2 = qr2, p3 = qr3;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const double u3 = u30 + t;
+                double g0 = vv[0][t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
+                if constexpr (DERIV != 0) {
+                    const double z1 = vv[1][t], z2 = vv[2][t], z3 = vv[3][t];
+                    g0 = fma(z1, p1, fma(z2, p2, fma(z3, p3, g0)));
+                    g1 = g * z1; g2 = g * z2; g3 = g * z3;
+                    p1 -= 2.0 * q[4]; p2 -= 2.0 * q[5]; p3 -= 2.0 * q[2];
+                }
+                g0 *= g;
+                double pw = 1.0;
+#pragma unroll
+                for (int kz = 0; kz <= L; kz++) {
+                    if (kz == 0) {
+                        A0[0] += g0;
+                        if (DERIV && L > 0) { A1[0] += g1; A2[0] += g2; A3[0] += g3; }
+                    } else {
+                        A0[kz] = fma(g0, pw, A0[kz]);
+                        if (DERIV && kz < L) { A1[kz] = fma(g1, pw, A1[kz]); A2[kz] = fma(g2, pw, A2[kz]); A3[kz] = fma(g3, pw, A3[kz]); }
+                    }
+                    if (kz < L) pw = kz == 0 ? u3 : pw * u3;
+                }
+                g *= r; r *= c33;
+            }
         }
-        grow *= r2; r2 *= c22; r3row *= c23;
         if (DERIV) {
-            qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5];
 #pragma unroll
-            for (int kz = 1; kz <= L; kz++) A0[kz] += kz * A3[kz - 1];
+            for (int kz = 1; kz <= L; kz++) A0[kz] = fma((double)kz, A3[kz - 1], A0[kz]);
         }
+        // powers of u2 (ORTHO: times the row's Gaussian factor)
         double pw2[L + 1];
-        pw2[0] = 1.0;
+        pw2[0] = ORTHO ? grow : 1.0;
 #pragma unroll
-        for (int k = 1; k <= L; k++) pw2[k] = k == 1 ? u2 : pw2[k - 1] * u2;
+        for (int k = 1; k <= L; k++) pw2[k] = (k == 1 && !ORTHO) ? u2 : pw2[k - 1] * u2;
 #pragma unroll
         for (int kz = 0; kz <= L; kz++)
 #pragma unroll
             for (int ky = 0; ky <= L - kz; ky++) {
-                if (ky == 0) B0[bidx(L, 0, kz)] += A0[kz];
-                else B0[bidx(L, ky, kz)] += A0[kz] * pw2[ky];
-                if (DERIV && ky > 0) B0[bidx(L, ky, kz)] += A2[kz] * (ky * pw2[ky - 1]);
+                if (ky == 0 && !ORTHO) B0[bidx(L, 0, kz)] += A0[kz];
+                else B0[bidx(L, ky, kz)] = fma(A0[kz], pw2[ky], B0[bidx(L, ky, kz)]);
+                if (DERIV && ky > 0) B0[bidx(L, ky, kz)] = fma(A2[kz], ky * pw2[ky - 1], B0[bidx(L, ky, kz)]);
                 if (DERIV && ky + kz <= L - 1) {
-                    if (ky == 0) B1[bidx(L - 1, 0, kz)] += A1[kz];
-                    else B1[bidx(L - 1, ky, kz)] += A1[kz] * pw2[ky];
+                    if (ky == 0 && !ORTHO) B1[bidx(L - 1, 0, kz)] += A1[kz];
+                    else B1[bidx(L - 1, ky, kz)] = fma(A1[kz], pw2[ky], B1[bidx(L - 1, ky, kz)]);
                 }
             }
+        grow *= r2; r2 *= c22;
+        if constexpr (!ORTHO) r3row *= c23;
+        if (DERIV) {
+            if constexpr (ORTHO) { qr2 -= 2.0 * q[1]; }
+            else { qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5]; }
+        }
     }
 }
 
@@ -426,8 +514,8 @@ GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, doubl
     for (int i = 0; i < NB; i++) B0[i] = 0.0;
 #pragma unroll
     for (int i = 0; i < NBX; i++) B1[i] = 0.0;
-    const SlabGauss SG = slab_gauss(q, u1, u20, u30);
-    integ_slab_rows<L, DERIV>([&](int k, int j, double *o) {
+    const SlabGauss SG = slab_gauss<false>(q, u1, u20, u30);
+    integ_slab_rows<L, DERIV, false>([&](int k, int j, double *o) {
         for (int t = 0; t < 4; t++) o[t] = v[k][j * 4 + t];
     }, q, c22, c23, c33, SG, u1, u20, u30, B0, B1);
     double pw1[L + 1];

@@ -31,7 +31,7 @@ struct BrickCtx {
     int x;                   // lane within the group = n1 plane
 };
 
-template <int L, int DERIV>
+template <int L, int DERIV, bool ORTHO>
 __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const PairRec pr, bool valid,
                                             double *__restrict__ mom) {
     constexpr int NCOMP = DERIV ? 4 : 1;
@@ -55,8 +55,8 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
         const int t2 = bit / BR3, t3 = bit - t2 * BR3;
         const double *chunk = c.vs + (bit * 4 + c.x) * CHS;
         const double u20 = u2b + 4 * t2, u30 = u3b + 4 * t3;
-        const SlabGauss SG = slab_gauss(q, u1, u20, u30);
-        integ_slab_rows<L, DERIV>(
+        const SlabGauss SG = slab_gauss<ORTHO>(q, u1, u20, u30);
+        integ_slab_rows<L, DERIV, ORTHO>(
             [&](int k, int j, double *o) {
                 const double2 a = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4);
                 const double2 b = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4 + 2);
@@ -85,7 +85,7 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
             }
 }
 
-template <int DERIV, int LMAX>
+template <int DERIV, int LMAX, bool ORTHO>
 __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
                                                                           const TaskK *__restrict__ tasks,
                                                                           const BEntry *__restrict__ entries,
@@ -184,43 +184,47 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
         have = next_chunk();
         if (have && base + grp < hi) { en = ent[base + grp]; pr = load_pair(tasks, en.task); }   // in flight during this chunk
         switch (Lc) {
-            case 0: integ_entry<0, DERIV>(c, enc, prc, valid, mom); break;
-            case 1: integ_entry<1, DERIV>(c, enc, prc, valid, mom); break;
-            case 2: integ_entry<2, DERIV>(c, enc, prc, valid, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV>(c, enc, prc, valid, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV>(c, enc, prc, valid, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV>(c, enc, prc, valid, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV>(c, enc, prc, valid, mom); break;
+            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
         }
     }
 }
 
-template <int DERIV, int LMAX>
+template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    double *mom, cudaStream_t st) {
     constexpr int smem = BRICK_TILES * 4 * chunk_doubles(DERIV ? 4 : 1) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
-        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    k_integrate<DERIV, LMAX><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, mom);
+    k_integrate<DERIV, LMAX, ORTHO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, mom);
     return cudaGetLastError();
+}
+
+template <int DERIV, bool ORTHO>
+cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
+                     double *mom, int max_L, cudaStream_t st) {
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, entries, items, nitem, mom, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, entries, items, nitem, mom, st);
+    return launch<DERIV, 6, ORTHO>(P, tasks, entries, items, nitem, mom, st);
 }
 
 }  // namespace
 
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, double *mom, int deriv, int max_L, cudaStream_t st) {
-    if (deriv) {
-        if (max_L <= 2) return launch<1, 2>(P, tasks, entries, items, nitem, mom, st);
-        if (max_L <= 4) return launch<1, 4>(P, tasks, entries, items, nitem, mom, st);
-        return launch<1, 6>(P, tasks, entries, items, nitem, mom, st);
-    }
-    if (max_L <= 2) return launch<0, 2>(P, tasks, entries, items, nitem, mom, st);
-    if (max_L <= 4) return launch<0, 4>(P, tasks, entries, items, nitem, mom, st);
-    return launch<0, 6>(P, tasks, entries, items, nitem, mom, st);
+                             int nitem, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st) {
+    if (deriv) return ortho ? launch_l<1, true>(P, tasks, entries, items, nitem, mom, max_L, st)
+                            : launch_l<1, false>(P, tasks, entries, items, nitem, mom, max_L, st);
+    return ortho ? launch_l<0, true>(P, tasks, entries, items, nitem, mom, max_L, st)
+                 : launch_l<0, false>(P, tasks, entries, items, nitem, mom, max_L, st);
 }
 
 }  // namespace gpw

@@ -215,6 +215,11 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
             build_S(g.H, hp->S[a]);
         }
+        // orthogonal lattice vectors (exact zeros, e.g. a diagonal cell matrix): the kernels' ORTHO variants
+        hp->ortho = true;
+        for (int a = 0; a < nlevel; a++)
+            for (int k = 3; k < 6; k++)
+                if (hp->lev[a].Gm[k] != 0.0) hp->ortho = false;
 
         // ---- T1 radii ----
         std::vector<double> prad(nprim, 0.0);
