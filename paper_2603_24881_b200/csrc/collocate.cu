@@ -6,84 +6,88 @@
 // points (gpw_math.cuh, colloc_slab).  Every lane keeps its rho values (and, for DERIV, the gradient in
 // grid-index components) in registers for the whole list; the eight groups are summed by a shuffle
 // reduce-scatter and the block is written once (the theoretical minimum the paper aims at),
-// with no per-point cross-thread reduction (the bottleneck of Alg. 1 l.11).  The next
-// visit's pair record and polynomial are copied to shared memory with cp.async while the current visit
-// is evaluated (two slots per group).
+// with no per-point cross-thread reduction (the bottleneck of Alg. 1 l.11).
+//
+// Data movement: the item's visits are cut into chunks of eight (one per group) that never straddle an L
+// segment; the chunk table is built once per item in shared memory.  A pair's record and polynomial are
+// one contiguous block of the workspace (8 + ncoef_pad(L) doubles) and reach the group's shared-memory
+// slot by cp.async (16 bytes per lane and trip) issued two chunks ahead; the item's visit records are copied
+// to shared memory once, so that no prefetched value waits in registers (the accumulators take 128 of the
+// 255 registers of the GGA variant; a bulk-copy version was measured slower: cp.async.bulk is a
+// warp-uniform instruction, eight different sources per chunk serialise).
 #include "gpw_kernels.cuh"
 
 namespace gpw {
 namespace {
 
-constexpr int NGRP = 8;   // groups of 4 lanes per warp
-constexpr int NWARP = 4;  // warps (work items) per CTA
+constexpr int NGRP = 8;     // groups of 4 lanes per warp
+constexpr int NWARP = 4;    // warps (work items) per CTA
+constexpr int NSLOT = 3;    // shared-memory slots per group (copy issued two chunks ahead)
+constexpr int MAXCH = 64;   // chunks per item: ITEM_MAX / NGRP full ones + one ragged chunk per L segment
+constexpr int MAXVIS = 384; // visits per item (ITEM_MAX of plan.cpp)
 
 // Shared-memory slot of one visit: the pair record (8 doubles) followed by the pair polynomial.
 GPW_CX int slot_doubles(int lmax) { return 8 + ncoef_pad(lmax); }
-// A group's two slots, padded so that consecutive groups start 16 bytes apart modulo the 128-byte bank
-// row: the eight groups' broadcast reads of the same coefficient then hit eight different bank pairs.
+// A group's slots, padded to an odd number of 16-byte units: the eight groups' broadcast reads of the same
+// coefficient then hit eight different bank pairs.
 GPW_CX int group_stride(int lmax) {
-    int n = 2 * slot_doubles(lmax);
-    while (n % 16 != 2) n += 2;
+    int n = NSLOT * slot_doubles(lmax);
+    while (n % 4 != 2) n += 2;
     return n;
 }
+// per warp: the groups' slots, the chunk table, the item's visit records
+GPW_CX int warp_doubles(int lmax) { return NGRP * group_stride(lmax) + MAXCH + MAXVIS; }
 
 struct ColCtx {
-    const TaskK *tasks;
-    const Visit *visits;   // already offset to the block's list
-    const double *work;    // pair polynomials
+    const double *rec;     // per-pair records: header (8 doubles) + polynomial
     const double *gm;      // the level's metric Gm (constant bank)
-    const long long *coef_base;   // the level's class offsets into the workspace (constant bank)
-    double *slot;          // the group's two shared-memory slots
+    const long long *coef_base;   // the level's class offsets (constant bank): record of pair i of class L
+                                  // starts at coef_base[L] + i * (8 + ncoef_pad(L))
+    double *slot;          // the group's shared-memory slots
     int n1, n2, n3;        // stored index of the lane's slab corner
     int N0, N1, N2;
     int x;                 // lane within the group
 };
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(unsigned smem, const void *gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem), "l"(gmem) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async8(unsigned smem, const void *gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// The group's four lanes copy the pair record and polynomial of `task` (class L) into a slot (16 bytes per
-// lane and trip).
-__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, double *slot) {
-    const int npad = ncoef_pad(L);
-    const int nch = 4 + npad / 2;   // 16-byte chunks
-    const char *src_k = reinterpret_cast<const char *>(c.tasks + task);
-    const char *src_c = reinterpret_cast<const char *>(c.work + c.coef_base[L] + (long long)task * npad);
-    for (int k = c.x; k < nch; k += 4)
-        cp_async16(reinterpret_cast<char *>(slot) + 16 * k, k < 4 ? src_k + 16 * k : src_c + 16 * (k - 4));
-    cp_async_commit();
+// A visit record is its raw 8 bytes: task in the low word, the three signed wrap counts in bytes 4..6.
+__device__ __forceinline__ int visit_task(unsigned long long r) { return (int)(unsigned)r; }
+__device__ __forceinline__ int visit_wrap(unsigned long long r, int axis) {
+    return (int)(signed char)(unsigned char)(r >> (32 + 8 * axis));
 }
 
-// The item's visits in chunks of NGRP that never straddle an L segment (so the code path is warp-uniform).
-// Lane l holds seg[l & 7] of the block; all lanes advance together.
-struct ChunkIt {
-    int L;
-    unsigned base, hi;   // the chunk is [base, min(base + NGRP, hi)); hi = end of the segment inside the item
-};
+// The group's four lanes copy the record of `task` (class L) into a slot, 16 bytes per lane and trip.
 template <int LMAX>
-__device__ __forceinline__ bool next_chunk(ChunkIt &it, unsigned it_lo, unsigned it_hi, unsigned myseg) {
-    it.base += NGRP;
-    while (it.L < 0 || it.base >= it.hi) {
-        it.L++;
-        if (it.L > LMAX) return false;
-        it.base = max(it_lo, __shfl_sync(0xffffffffu, myseg, it.L));
-        it.hi = min(it_hi, __shfl_sync(0xffffffffu, myseg, it.L + 1));
-    }
-    return true;
+__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, double *slot) {
+    const int nrec = 8 + ncoef_pad(L);          // doubles, even
+    const char *src = reinterpret_cast<const char *>(c.rec + c.coef_base[L] + (long long)task * nrec) + 16 * c.x;
+    const unsigned dst = smem_u32(slot) + 16 * c.x;
+    const int n16 = nrec / 2 - c.x;             // 16-byte units left for this lane, stride 4
+    constexpr int TRIPS = (slot_doubles(LMAX) / 2 + 3) / 4;
+#pragma unroll
+    for (int t = 0; t < TRIPS; t++)
+        if (4 * t < n16) cp_async16(dst + 64 * t, src + 64 * t);
 }
 
 template <int L, int DERIV, bool ORTHO>
-__device__ __forceinline__ void colloc_visit(const ColCtx &c, const Visit vi, const double *s, double (*acc)[16]) {
+__device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long vi, const double *s, double (*acc)[16]) {
     const double ap = s[3];
     double q[6];
 #pragma unroll
     for (int k = 0; k < 6; k++) q[k] = ap * c.gm[k];
-    const double u1 = (double)(c.n1 + vi.s[0] * c.N0) - s[0];
-    const double u20 = (double)(c.n2 + vi.s[1] * c.N1) - s[1];
-    const double u30 = (double)(c.n3 + vi.s[2] * c.N2) - s[2];
+    const double u1 = (double)(c.n1 + visit_wrap(vi, 0) * c.N0) - s[0];
+    const double u20 = (double)(c.n2 + visit_wrap(vi, 1) * c.N1) - s[1];
+    const double u30 = (double)(c.n3 + visit_wrap(vi, 2) * c.N2) - s[2];
     colloc_slab<L, DERIV, ORTHO>(s + 8, q, s[4], s[5], s[6], u1, u20, u30, acc);
 }
 
@@ -110,32 +114,59 @@ __device__ __forceinline__ int group_reduce_scatter(double *a, int lane) {
 
 template <int DERIV, int LMAX, bool ORTHO>
 __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_constant__ GridParams P,
-                                                                   const TaskK *__restrict__ tasks,
                                                                    const Visit *__restrict__ visits,
                                                                    const Item *__restrict__ items, int nitem,
-                                                                   const double *__restrict__ coef) {
+                                                                   const double *__restrict__ rec) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int SLOT = slot_doubles(LMAX);
     constexpr int GSTRIDE = group_stride(LMAX);
-    extern __shared__ __align__(16) double sm[];   // [NWARP][NGRP] x (two slots, padded to GSTRIDE)
-    const int w = blockIdx.x * NWARP + (threadIdx.x >> 5);
+    extern __shared__ __align__(16) double sm[];
+    const int warp = threadIdx.x >> 5;
+    const int w = blockIdx.x * NWARP + warp;
     if (w >= nitem) return;
     const Item it = items[w];
     const LevelGeom &g = P.lev[it.level];
     const int lane = threadIdx.x & 31, grp = lane >> 2, x = lane & 3;
-    const int T2 = g.T[2], T1 = g.T[1];
-    const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
+    double *wsm = sm + (size_t)warp * warp_doubles(LMAX);
+    uint2 *tab = reinterpret_cast<uint2 *>(wsm + NGRP * GSTRIDE);
+    unsigned long long *vis = reinterpret_cast<unsigned long long *>(wsm + NGRP * GSTRIDE + MAXCH);
+
+    // ---- the item's visit records -> shared memory (first cp.async group) ----
+    {
+        const Visit *src = visits + P.tile_base[it.level][it.tile] + it.lo;
+        const int n = min((int)(it.hi - it.lo), MAXVIS);   // cannot bind: items have at most MAXVIS visits
+        for (int i = lane; i < n; i += 32) cp_async8(smem_u32(vis + i), src + i);
+        cp_async_commit();
+    }
+    // ---- chunk table: entry = (first visit relative to it.lo, L | visits << 8) ----
+    const unsigned myseg = P.seg[it.level][(size_t)it.tile * 8 + (lane & 7)];
+    int nch = 0;
+#pragma unroll 1
+    for (int L = 0; L <= LMAX; L++) {
+        const unsigned lo = max(it.lo, __shfl_sync(0xffffffffu, myseg, L));
+        const unsigned hi = min(it.hi, __shfl_sync(0xffffffffu, myseg, L + 1));
+        if (lo >= hi) continue;
+        const int n = (int)((hi - lo + NGRP - 1) / NGRP);
+        for (int k = lane; k < n; k += 32) {
+            const unsigned base = lo + NGRP * k;
+            if (nch + k < MAXCH) tab[nch + k] = make_uint2(base - it.lo, (unsigned)L | (min(hi - base, (unsigned)NGRP) << 8));
+        }
+        nch += n;
+    }
+    nch = min(nch, MAXCH);   // cannot bind: at most MAXVIS / NGRP full chunks + one ragged chunk per L segment
+
     ColCtx c;
-    c.tasks = tasks;
-    c.visits = visits + P.tile_base[it.level][it.tile];
-    c.work = coef;
+    c.rec = rec;
     c.gm = g.Gm;
     c.coef_base = P.coef_base[it.level];
-    c.slot = sm + (size_t)((threadIdx.x >> 5) * NGRP + grp) * GSTRIDE;
+    c.slot = wsm + (size_t)grp * GSTRIDE;
     c.x = x;
-    c.n1 = 4 * b1 + x; c.n2 = 4 * b2; c.n3 = 4 * b3;
+    {
+        const int T2 = g.T[2], T1 = g.T[1];
+        const int b3 = it.tile % T2, b2 = (it.tile / T2) % T1, b1 = it.tile / (T2 * T1);
+        c.n1 = 4 * b1 + x; c.n2 = 4 * b2; c.n3 = 4 * b3;
+    }
     c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
-    const unsigned myseg = P.seg[it.level][(size_t)it.tile * 8 + (lane & 7)];
 
     double acc[NCOMP][16];
 #pragma unroll
@@ -143,30 +174,32 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 #pragma unroll
         for (int i = 0; i < 16; i++) acc[k][i] = 0.0;
 
-    // Software pipeline over the chunks, across L segments: the visit records of chunk k+2 are loaded and
-    // the pair record + polynomial of chunk k+1 are copied to shared memory (cp.async) while chunk k is
-    // evaluated.
-    ChunkIt c0{-1, 0u, 0u};
-    bool h0 = next_chunk<LMAX>(c0, it.lo, it.hi, myseg);
-    ChunkIt c1 = c0;
-    bool h1 = h0 && next_chunk<LMAX>(c1, it.lo, it.hi, myseg);
-    Visit v0, v1;
-    v0.task = 0; v0.s[0] = v0.s[1] = v0.s[2] = 0; v0.pad = 0;
-    v1 = v0;
-    if (h0 && c0.base + grp < c0.hi) { v0 = c.visits[c0.base + grp]; stage_visit(c, c0.L, v0.task, c.slot); }
-    if (h1 && c1.base + grp < c1.hi) v1 = c.visits[c1.base + grp];
-    int cur = 0;
-    while (h0) {
-        ChunkIt c2 = c1;
-        const bool h2 = h1 && next_chunk<LMAX>(c2, it.lo, it.hi, myseg);
-        Visit v2 = v1;
-        if (h2 && c2.base + grp < c2.hi) v2 = c.visits[c2.base + grp];
-        cp_async_wait_all();
-        __syncwarp();   // the slot is complete, and every lane has left the slot refilled next
-        if (h1 && c1.base + grp < c1.hi) stage_visit(c, c1.L, v1.task, c.slot + (cur ^ 1) * SLOT);
-        if (c0.base + grp < c0.hi) {
-            const double *s = c.slot + cur * SLOT;
-            switch (c0.L) {
+    cp_async_wait<0>();
+    __syncwarp();   // visit records and chunk table complete
+
+    // ---- software pipeline over the chunks: the records of chunk k+2 are in flight while chunk k is evaluated;
+    //      one commit group per chunk (empty past the end), so "all but the newest" = chunks <= k complete ----
+    auto stage_chunk = [&](int k, int slot) {
+        if (k < nch) {
+            const uint2 e = tab[k];
+            if ((unsigned)grp < (e.y >> 8))
+                stage_visit<LMAX>(c, (int)(e.y & 0xffu), visit_task(vis[e.x + grp]), c.slot + slot * SLOT);
+        }
+        cp_async_commit();
+    };
+    stage_chunk(0, 0);
+    stage_chunk(1, 1);
+    int slot = 0;
+#pragma unroll 1
+    for (int k = 0; k < nch; k++) {
+        cp_async_wait<1>();   // chunk k has landed (chunk k+1 may still be in flight)
+        __syncwarp();         // ... for all four lanes of the group; and every lane has left the slot refilled next
+        stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
+        const uint2 e = tab[k];
+        if ((unsigned)grp < (e.y >> 8)) {
+            const unsigned long long v0 = vis[e.x + grp];
+            const double *s = c.slot + slot * SLOT;
+            switch ((int)(e.y & 0xffu)) {
                 case 0: colloc_visit<0, DERIV, ORTHO>(c, v0, s, acc); break;
                 case 1: colloc_visit<1, DERIV, ORTHO>(c, v0, s, acc); break;
                 case 2: colloc_visit<2, DERIV, ORTHO>(c, v0, s, acc); break;
@@ -176,10 +209,9 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
                 default: if constexpr (LMAX >= 6) colloc_visit<6, DERIV, ORTHO>(c, v0, s, acc); break;
             }
         }
-        c0 = c1; h0 = h1; v0 = v1;
-        c1 = c2; h1 = h2; v1 = v2;
-        cur ^= 1;
+        if (++slot == NSLOT) slot = 0;
     }
+    cp_async_wait<0>();
     __syncwarp();
     // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i (linear: before the sum)
     if constexpr (DERIV != 0) {
@@ -211,35 +243,35 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 }
 
 template <int DERIV, int LMAX, bool ORTHO>
-cudaError_t launch(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items, int nitem,
-                   const double *coef, cudaStream_t st) {
-    constexpr int smem = NWARP * NGRP * group_stride(LMAX) * (int)sizeof(double);
+cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                   const double *rec, cudaStream_t st) {
+    constexpr int smem = NWARP * warp_doubles(LMAX) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
         const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, tasks, visits, items, nitem, coef);
+    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec);
     return cudaGetLastError();
 }
 
 template <int DERIV, bool ORTHO>
-cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items, int nitem,
-                     const double *coef, int max_L, cudaStream_t st) {
-    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, visits, items, nitem, coef, st);
-    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, visits, items, nitem, coef, st);
-    return launch<DERIV, 6, ORTHO>(P, tasks, visits, items, nitem, coef, st);
+cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                     const double *rec, int max_L, cudaStream_t st) {
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, visits, items, nitem, rec, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, visits, items, nitem, rec, st);
+    return launch<DERIV, 6, ORTHO>(P, visits, items, nitem, rec, st);
 }
 
 }  // namespace
 
-cudaError_t launch_collocate(const GridParams &P, const TaskK *tasks, const Visit *visits, const Item *items,
-                             int nitem, const double *coef, int deriv, int max_L, bool ortho, cudaStream_t st) {
-    if (deriv) return ortho ? launch_l<1, true>(P, tasks, visits, items, nitem, coef, max_L, st)
-                            : launch_l<1, false>(P, tasks, visits, items, nitem, coef, max_L, st);
-    return ortho ? launch_l<0, true>(P, tasks, visits, items, nitem, coef, max_L, st)
-                 : launch_l<0, false>(P, tasks, visits, items, nitem, coef, max_L, st);
+cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                             const double *rec, int deriv, int max_L, bool ortho, cudaStream_t st) {
+    if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, rec, max_L, st)
+                            : launch_l<1, false>(P, visits, items, nitem, rec, max_L, st);
+    return ortho ? launch_l<0, true>(P, visits, items, nitem, rec, max_L, st)
+                 : launch_l<0, false>(P, visits, items, nitem, rec, max_L, st);
 }
 
 }  // namespace gpw

@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -24,7 +25,8 @@ __global__ void __launch_bounds__(128) k_poly_from_D(const TaskP *__restrict__ t
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntask) return;
     const TaskP p = tp[t];
-    pair_poly_from_D(p, D, nao, S_all + (size_t)p.level * S_TOTAL, coef + p.coef_off);
+    // the pair's record in the collocation workspace: 8-double header, then the polynomial
+    pair_poly_from_D(p, D, nao, S_all + (size_t)p.level * S_TOTAL, coef + p.coef_off + 8 * (long long)t + 8);
 }
 
 struct DVs { double v[GPW_MAX_LEVEL]; };
@@ -85,7 +87,7 @@ struct gpw_plan {
     double *d_S = nullptr;
     long long *d_tile_base[GPW_MAX_LEVEL] = {nullptr};
     unsigned *d_seg[GPW_MAX_LEVEL] = {nullptr};
-    double *d_coef = nullptr;   // polynomial workspace of gpw_eval_rho
+    double *d_coef = nullptr;   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
     double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
     // optional kernel timing (gpw_plan_set_timing): events around each kernel of the last eval calls
     bool timing = false;
@@ -182,9 +184,19 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
         ok = ok && upload(&p->d_brick_base[a], hp->brick_base[a].data(), hp->brick_base[a].size(), nb, "upload brick offsets");
     }
     const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
-    ok = ok && cuda_ok(cudaMalloc((void **)&p->d_coef, sizeof(double) * nw), "allocate polynomial workspace");
+    if (ok) {
+        // collocation records: [nP0 nP1 nP2 a_p c22 c23 c33 c11 | polynomial] per pair, headers written once
+        std::vector<double> rec(nw + 8 * hp->taskK.size(), 0.0);
+        for (size_t i = 0; i < hp->taskK.size(); i++) {
+            const TaskK &k = hp->taskK[i];
+            double *h = rec.data() + k.coef_off + 8 * (long long)i;
+            h[0] = k.nP[0]; h[1] = k.nP[1]; h[2] = k.nP[2]; h[3] = k.ap; h[4] = k.c22; h[5] = k.c23; h[6] = k.c33;
+            h[7] = std::exp(-2.0 * k.ap * hp->lev[hp->task[i].level].Gm[0]);
+        }
+        ok = upload(&p->d_coef, rec.data(), rec.size(), nb, "upload pair records");
+    }
     ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
-    if (ok) nb += (long)(2 * sizeof(double) * nw);
+    if (ok) nb += (long)(sizeof(double) * nw);
     if (!ok) {
         free_device(p);
         delete hp;
@@ -261,7 +273,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->d_taskK, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, hp->ortho, st),
+    if (!cuda_ok(launch_collocate(P, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
