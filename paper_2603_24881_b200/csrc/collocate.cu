@@ -26,20 +26,26 @@ constexpr int NSLOT = 3;    // shared-memory slots per group (copy issued two ch
 constexpr int MAXCH = 64;   // chunks per item: ITEM_MAX / NGRP full ones + one ragged chunk per L segment
 constexpr int MAXVIS = 384; // visits per item (ITEM_MAX of plan.cpp)
 
-// Shared-memory slot of one visit: the pair record (8 doubles) followed by the pair polynomial.
-GPW_CX int slot_doubles(int lmax) { return 8 + ncoef_pad(lmax); }
+// Per-visit Gaussian values (k_visit_gauss, computed once per plan: they depend on the geometry only): the
+// Gaussian at the corner of each of the four lanes' slabs and the first-step ratios along n2 and n3, which for
+// orthogonal lattice vectors are the same for the four slabs.
+GPW_CX int vg_doubles(bool ortho) { return ortho ? 6 : 12; }
+// Shared-memory slot of one visit: the pair record (8 doubles), the pair polynomial, the visit's Gaussian values.
+GPW_CX int slot_vg(int lmax) { return 8 + ncoef_pad(lmax); }
+GPW_CX int slot_doubles(int lmax, bool ortho) { return slot_vg(lmax) + vg_doubles(ortho); }
 // A group's slots, padded to an odd number of 16-byte units: the eight groups' broadcast reads of the same
 // coefficient then hit eight different bank pairs.
-GPW_CX int group_stride(int lmax) {
-    int n = NSLOT * slot_doubles(lmax);
+GPW_CX int group_stride(int lmax, bool ortho) {
+    int n = NSLOT * slot_doubles(lmax, ortho);
     while (n % 4 != 2) n += 2;
     return n;
 }
 // per warp: the groups' slots, the chunk table, the item's visit records
-GPW_CX int warp_doubles(int lmax) { return NGRP * group_stride(lmax) + MAXCH + MAXVIS; }
+GPW_CX int warp_doubles(int lmax, bool ortho) { return NGRP * group_stride(lmax, ortho) + MAXCH + MAXVIS; }
 
 struct ColCtx {
     const double *rec;     // per-pair records: header (8 doubles) + polynomial
+    const double *vg;      // Gaussian values of the item's visits (vg_doubles per visit)
     const double *gm;      // the level's metric Gm (constant bank)
     const long long *coef_base;   // the level's class offsets (constant bank): record of pair i of class L
                                   // starts at coef_base[L] + i * (8 + ncoef_pad(L))
@@ -67,19 +73,25 @@ __device__ __forceinline__ int visit_wrap(unsigned long long r, int axis) {
 }
 
 // The group's four lanes copy the record of `task` (class L) into a slot, 16 bytes per lane and trip.
-template <int LMAX>
-__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, double *slot) {
+// ... and the visit's Gaussian values (visit index iv relative to the item's first visit).
+template <int LMAX, bool ORTHO>
+__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, unsigned iv, double *slot) {
     const int nrec = 8 + ncoef_pad(L);          // doubles, even
     const char *src = reinterpret_cast<const char *>(c.rec + c.coef_base[L] + (long long)task * nrec) + 16 * c.x;
     const unsigned dst = smem_u32(slot) + 16 * c.x;
     const int n16 = nrec / 2 - c.x;             // 16-byte units left for this lane, stride 4
-    constexpr int TRIPS = (slot_doubles(LMAX) / 2 + 3) / 4;
+    constexpr int TRIPS = (slot_vg(LMAX) / 2 + 3) / 4;
 #pragma unroll
     for (int t = 0; t < TRIPS; t++)
         if (4 * t < n16) cp_async16(dst + 64 * t, src + 64 * t);
+    constexpr int VG = vg_doubles(ORTHO);
+    const char *gsrc = reinterpret_cast<const char *>(c.vg + (size_t)iv * VG) + 16 * c.x;
+    const unsigned gdst = smem_u32(slot + slot_vg(LMAX)) + 16 * c.x;
+    if (c.x < VG / 2) cp_async16(gdst, gsrc);
+    if constexpr (VG / 2 > 4) { if (c.x + 4 < VG / 2) cp_async16(gdst + 64, gsrc + 64); }
 }
 
-template <int L, int DERIV, bool ORTHO>
+template <int L, int LMAX, int DERIV, bool ORTHO>
 __device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long vi, const double *s, double (*acc)[16]) {
     const double ap = s[3];
     double q[6];
@@ -88,7 +100,12 @@ __device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long
     const double u1 = (double)(c.n1 + visit_wrap(vi, 0) * c.N0) - s[0];
     const double u20 = (double)(c.n2 + visit_wrap(vi, 1) * c.N1) - s[1];
     const double u30 = (double)(c.n3 + visit_wrap(vi, 2) * c.N2) - s[2];
-    colloc_slab<L, DERIV, ORTHO>(s + 8, q, s[4], s[5], s[6], u1, u20, u30, acc);
+    const double *gv = s + slot_vg(LMAX);
+    SlabGauss SG;
+    SG.g0 = gv[c.x];
+    SG.r2 = ORTHO ? gv[4] : gv[4 + c.x];
+    SG.r3 = ORTHO ? gv[5] : gv[8 + c.x];
+    colloc_slab<L, DERIV, ORTHO>(s + 8, q, s[4], s[5], s[6], SG, u1, u20, u30, acc);
 }
 
 // Sum an N-vector over the eight groups (lane bits 4, 8, 16); afterwards the lane holds N/8 sums,
@@ -116,10 +133,11 @@ template <int DERIV, int LMAX, bool ORTHO>
 __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_constant__ GridParams P,
                                                                    const Visit *__restrict__ visits,
                                                                    const Item *__restrict__ items, int nitem,
-                                                                   const double *__restrict__ rec) {
+                                                                   const double *__restrict__ rec,
+                                                                   const double *__restrict__ vg) {
     constexpr int NCOMP = DERIV ? 4 : 1;
-    constexpr int SLOT = slot_doubles(LMAX);
-    constexpr int GSTRIDE = group_stride(LMAX);
+    constexpr int SLOT = slot_doubles(LMAX, ORTHO);
+    constexpr int GSTRIDE = group_stride(LMAX, ORTHO);
     extern __shared__ __align__(16) double sm[];
     const int warp = threadIdx.x >> 5;
     const int w = blockIdx.x * NWARP + warp;
@@ -127,7 +145,7 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
     const Item it = items[w];
     const LevelGeom &g = P.lev[it.level];
     const int lane = threadIdx.x & 31, grp = lane >> 2, x = lane & 3;
-    double *wsm = sm + (size_t)warp * warp_doubles(LMAX);
+    double *wsm = sm + (size_t)warp * warp_doubles(LMAX, ORTHO);
     uint2 *tab = reinterpret_cast<uint2 *>(wsm + NGRP * GSTRIDE);
     unsigned long long *vis = reinterpret_cast<unsigned long long *>(wsm + NGRP * GSTRIDE + MAXCH);
 
@@ -157,6 +175,7 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 
     ColCtx c;
     c.rec = rec;
+    c.vg = vg + (size_t)(P.tile_base[it.level][it.tile] + it.lo) * vg_doubles(ORTHO);
     c.gm = g.Gm;
     c.coef_base = P.coef_base[it.level];
     c.slot = wsm + (size_t)grp * GSTRIDE;
@@ -183,7 +202,7 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
         if (k < nch) {
             const uint2 e = tab[k];
             if ((unsigned)grp < (e.y >> 8))
-                stage_visit<LMAX>(c, (int)(e.y & 0xffu), visit_task(vis[e.x + grp]), c.slot + slot * SLOT);
+                stage_visit<LMAX, ORTHO>(c, (int)(e.y & 0xffu), visit_task(vis[e.x + grp]), e.x + grp, c.slot + slot * SLOT);
         }
         cp_async_commit();
     };
@@ -200,13 +219,13 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
             const unsigned long long v0 = vis[e.x + grp];
             const double *s = c.slot + slot * SLOT;
             switch ((int)(e.y & 0xffu)) {
-                case 0: colloc_visit<0, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 1: colloc_visit<1, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 2: colloc_visit<2, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 3: if constexpr (LMAX >= 3) colloc_visit<3, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 4: if constexpr (LMAX >= 4) colloc_visit<4, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 5: if constexpr (LMAX >= 5) colloc_visit<5, DERIV, ORTHO>(c, v0, s, acc); break;
-                default: if constexpr (LMAX >= 6) colloc_visit<6, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 0: colloc_visit<0, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 1: colloc_visit<1, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 2: colloc_visit<2, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 3: if constexpr (LMAX >= 3) colloc_visit<3, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 4: if constexpr (LMAX >= 4) colloc_visit<4, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                case 5: if constexpr (LMAX >= 5) colloc_visit<5, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
+                default: if constexpr (LMAX >= 6) colloc_visit<6, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
             }
         }
         if (++slot == NSLOT) slot = 0;
@@ -244,34 +263,90 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 
 template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                   const double *rec, cudaStream_t st) {
-    constexpr int smem = NWARP * warp_doubles(LMAX) * (int)sizeof(double);
+                   const double *rec, const double *vg, cudaStream_t st) {
+    constexpr int smem = NWARP * warp_doubles(LMAX, ORTHO) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
         const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec);
+    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
     return cudaGetLastError();
 }
 
 template <int DERIV, bool ORTHO>
 cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                     const double *rec, int max_L, cudaStream_t st) {
-    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, visits, items, nitem, rec, st);
-    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, visits, items, nitem, rec, st);
-    return launch<DERIV, 6, ORTHO>(P, visits, items, nitem, rec, st);
+                     const double *rec, const double *vg, int max_L, cudaStream_t st) {
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, visits, items, nitem, rec, vg, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, visits, items, nitem, rec, vg, st);
+    return launch<DERIV, 6, ORTHO>(P, visits, items, nitem, rec, vg, st);
 }
 
 }  // namespace
 
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                             const double *rec, int deriv, int max_L, bool ortho, cudaStream_t st) {
-    if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, rec, max_L, st)
-                            : launch_l<1, false>(P, visits, items, nitem, rec, max_L, st);
-    return ortho ? launch_l<0, true>(P, visits, items, nitem, rec, max_L, st)
-                 : launch_l<0, false>(P, visits, items, nitem, rec, max_L, st);
+                             const double *rec, const double *vg, int deriv, int max_L, bool ortho, cudaStream_t st) {
+    if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, rec, vg, max_L, st)
+                            : launch_l<1, false>(P, visits, items, nitem, rec, vg, max_L, st);
+    return ortho ? launch_l<0, true>(P, visits, items, nitem, rec, vg, max_L, st)
+                 : launch_l<0, false>(P, visits, items, nitem, rec, vg, max_L, st);
+}
+
+// ---------------------------------------------------------------------------------------- plan-time kernel
+// Gaussian values of every (pair, block) visit, in the order of the visit lists: one CTA per stored block.
+//   ORTHO:  [G(x = 0..3), r2, r3]      else:  [G(x = 0..3), r2(x = 0..3), r3(x = 0..3)]
+// G(x) = exp(-a_p |H u|^2) at the corner (u10 + x, u20, u30) of lane x's slab, r2 / r3 = the ratio to the next
+// point along n2 / n3 there (the starting values of the recursion of Eq. 24-25).
+namespace {
+template <bool ORTHO>
+__global__ void __launch_bounds__(128) k_visit_gauss(const __grid_constant__ GridParams P, const TaskK *__restrict__ tasks,
+                                                     const Visit *__restrict__ visits, double *__restrict__ vg) {
+    constexpr int VG = vg_doubles(ORTHO);
+    int tile = blockIdx.x, level = 0;
+    while (tile >= P.lev[level].ntile) { tile -= P.lev[level].ntile; level++; }
+    const LevelGeom &g = P.lev[level];
+    const long long lo = P.tile_base[level][tile], hi = P.tile_base[level][tile + 1];
+    const int T2 = g.T[2], T1 = g.T[1];
+    const int n3 = 4 * (tile % T2), n2 = 4 * ((tile / T2) % T1), n1 = 4 * (tile / (T2 * T1));
+    for (long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        const Visit v = visits[i];
+        const TaskK k = tasks[v.task];
+        double q[6];
+#pragma unroll
+        for (int m = 0; m < 6; m++) q[m] = k.ap * g.Gm[m];
+        const double u10 = (double)(n1 + v.s[0] * g.N[0]) - k.nP[0];
+        const double u20 = (double)(n2 + v.s[1] * g.N[1]) - k.nP[1];
+        const double u30 = (double)(n3 + v.s[2] * g.N[2]) - k.nP[2];
+        double *o = vg + (size_t)i * VG;
+#pragma unroll
+        for (int x = 0; x < 4; x++) {
+            const double u1 = u10 + x;
+            if constexpr (ORTHO) {
+                o[x] = exp(-fma(q[0] * u1, u1, fma(q[1] * u20, u20, q[2] * u30 * u30)));
+            } else {
+                o[x] = exp(-(q[0] * u1 * u1 + q[1] * u20 * u20 + q[2] * u30 * u30 +
+                             2.0 * (q[3] * u1 * u20 + (q[4] * u1 + q[5] * u20) * u30)));
+                o[4 + x] = exp(-(2.0 * (q[3] * u1 + q[1] * u20 + q[5] * u30) + q[1]));
+                o[8 + x] = exp(-(2.0 * (q[4] * u1 + q[5] * u20 + q[2] * u30) + q[2]));
+            }
+        }
+        if constexpr (ORTHO) {
+            o[4] = exp(-(q[1] * fma(2.0, u20, 1.0)));
+            o[5] = exp(-(q[2] * fma(2.0, u30, 1.0)));
+        }
+    }
+}
+}  // namespace
+
+size_t visit_gauss_doubles(bool ortho) { return (size_t)vg_doubles(ortho); }
+
+cudaError_t launch_visit_gauss(const GridParams &P, int ntile_all, const TaskK *tasks, const Visit *visits, double *vg,
+                               bool ortho, cudaStream_t st) {
+    if (ntile_all <= 0) return cudaSuccess;
+    if (ortho) k_visit_gauss<true><<<ntile_all, 128, 0, st>>>(P, tasks, visits, vg);
+    else k_visit_gauss<false><<<ntile_all, 128, 0, st>>>(P, tasks, visits, vg);
+    return cudaGetLastError();
 }
 
 }  // namespace gpw

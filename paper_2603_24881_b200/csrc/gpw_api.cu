@@ -89,6 +89,7 @@ struct gpw_plan {
     unsigned *d_seg[GPW_MAX_LEVEL] = {nullptr};
     double *d_coef = nullptr;   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
     double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
+    double *d_vg = nullptr;     // Gaussian values of every (pair, block) visit (geometry only; written at build time)
     // optional kernel timing (gpw_plan_set_timing): events around each kernel of the last eval calls
     bool timing = false;
     cudaEvent_t ev[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
@@ -121,7 +122,7 @@ void free_device(gpw_plan *p) {
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
     cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_visit); cudaFree(p->d_item); cudaFree(p->d_S);
-    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_bentry); cudaFree(p->d_bitem);
+    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg); cudaFree(p->d_bentry); cudaFree(p->d_bitem);
     for (int a = 0; a < GPW_MAX_LEVEL; a++) cudaFree(p->d_brick_base[a]);
     for (int a = 0; a < GPW_MAX_LEVEL; a++) { cudaFree(p->d_tile_base[a]); cudaFree(p->d_seg[a]); }
 }
@@ -197,6 +198,21 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     }
     ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
     if (ok) nb += (long)(sizeof(double) * nw);
+    if (ok) {
+        const size_t nvg = hp->visit.size() * visit_gauss_doubles(hp->ortho);
+        ok = cuda_ok(cudaMalloc((void **)&p->d_vg, sizeof(double) * (nvg ? nvg : 1)), "allocate visit Gaussians");
+        if (ok) {
+            nb += (long)(sizeof(double) * nvg);
+            GridParams P;
+            double *none[GPW_MAX_LEVEL] = {nullptr};
+            fill_params(p, P, none);
+            int ntile_all = 0;
+            for (int a = 0; a < hp->nlevel; a++) ntile_all += hp->lev[a].ntile;
+            ok = hp->visit.empty() ||
+                 (cuda_ok(launch_visit_gauss(P, ntile_all, p->d_taskK, p->d_visit, p->d_vg, hp->ortho, 0), "visit Gaussians") &&
+                  cuda_ok(cudaDeviceSynchronize(), "visit Gaussians"));
+        }
+    }
     if (!ok) {
         free_device(p);
         delete hp;
@@ -273,7 +289,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->d_visit, p->d_item, nitem, p->d_coef, deriv, hp->max_L, hp->ortho, st),
+    if (!cuda_ok(launch_collocate(P, p->d_visit, p->d_item, nitem, p->d_coef, p->d_vg, deriv, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;

@@ -34,8 +34,13 @@ __device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, in
 // launchers (each picks the instantiation for the plan's largest L; ortho: every level's Gm is diagonal)
 // rec: per-pair records of the collocation kernel, header (8 doubles: nP[3], a_p, c22, c23, c33, c11) followed
 // by the pair polynomial; the record of pair i of class (level, L) starts at coef_base[level][L] + i * (8 + ncoef_pad(L))
+// vg: Gaussian values of every visit (visit_gauss_doubles(ortho) per visit, order of `visits`), written once per
+// plan by launch_visit_gauss
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                             const double *rec, int deriv, int max_L, bool ortho, cudaStream_t st);
+                             const double *rec, const double *vg, int deriv, int max_L, bool ortho, cudaStream_t st);
+size_t visit_gauss_doubles(bool ortho);
+cudaError_t launch_visit_gauss(const GridParams &P, int ntile_all, const TaskK *tasks, const Visit *visits, double *vg,
+                               bool ortho, cudaStream_t st);
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
                              int nitem, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st);
 

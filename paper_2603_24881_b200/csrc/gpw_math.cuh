@@ -6,10 +6,11 @@
 // with Q a polynomial of total degree L = la + lb.  A pre-pass expands Q about the Gaussian-product
 // centre P (binomial expansion, Eq. 26-27) and rewrites it in grid-index coordinates
 // u = n - n_P (r - P = H u, H = grid step matrix), which keeps one code path for orthorhombic and
-// non-orthogonal cells (the paper's A.30-A.33 split).  A thread owns a column of four
-// grid points along n3: stage A collapses the polynomial to a[kz](u1,u2), stage B is a Horner sweep in
-// u3.  The Gaussian along the column follows the recursion of Eq. (24)-(25).
-// Integration is the exact transpose: column moments, then outer products into the pair's moment vector.
+// non-orthogonal cells (the paper's A.30-A.33 split).  A lane owns a slab of 4 x 4 grid
+// points at its own n1: the polynomial is collapsed in u1 once per slab, in u2 once per row and swept by
+// Horner in u3 per point.  The Gaussian on the slab follows the recursion of Eq. (24)-(25)
+// from its value at the slab corner and two first-step ratios.  Integration is the exact transpose: row sums,
+// partial moments at fixed u1, then the expansion in u1.
 #pragma once
 #include "gpw_internal.h"
 
@@ -148,69 +149,6 @@ GPW_HD void pair_block_from_moments(const TaskP &p, const double *m, const doubl
     }
 }
 
-// Gaussian exp(-a_p |H u|^2) on the four points u3 = u30 + t of a column, by the two-term recursion of
-// Eq. (24)-(25) generalised to a non-orthogonal step matrix (cross terms of A.30-A.33 enter through the
-// slope).  q[6] = a_p * Gm (11 22 33 12 13 23), cc = exp(-2 q33).
-GPW_HD void column_gauss(const double *q, double cc, double u1, double u2, double u30, double *G) {
-    const double E0 = q[0] * u1 * u1 + q[1] * u2 * u2 + q[2] * u30 * u30 +
-                      2.0 * (q[3] * u1 * u2 + (q[4] * u1 + q[5] * u2) * u30);
-    const double sl = 2.0 * (q[4] * u1 + q[5] * u2 + q[2] * u30) + q[2];
-    double g = exp(-E0);
-    double r = exp(-sl);
-    G[0] = g;
-    g *= r; r *= cc; G[1] = g;
-    g *= r; r *= cc; G[2] = g;
-    g *= r; G[3] = g;
-}
-
-// Collocation of one pair on one column of four points.
-//   c      the pair's polynomial (cidx order), broadcast reads
-//   acc    [NCOMP][4] running sums; for DERIV the gradient is accumulated in grid-index coordinates
-//          (the constant map to Cartesian is applied once when the block is written)
-template <int L, int DERIV>
-GPW_HD void colloc_column(const double *__restrict__ c, const double *q, double cc, double u1, double u2,
-                          double u30, double (*acc)[4]) {
-    double a[L + 1], ax[L + 1], ay[L + 1];
-#pragma unroll
-    for (int kz = 0; kz <= L; kz++) {
-        double s = 0.0, sx = 0.0, sy = 0.0;
-#pragma unroll
-        for (int ky = L - kz; ky >= 0; ky--) {
-            double p = 0.0, dp = 0.0;
-#pragma unroll
-            for (int kx = L - kz - ky; kx >= 0; kx--) {
-                if (DERIV) dp = dp * u1 + p;
-                p = p * u1 + c[cidx(L, kx, ky, kz)];
-            }
-            if (DERIV) { sy = sy * u2 + s; sx = sx * u2 + dp; }
-            s = s * u2 + p;
-        }
-        a[kz] = s; ax[kz] = sx; ay[kz] = sy;
-    }
-    double G[4];
-    column_gauss(q, cc, u1, u2, u30, G);
-#pragma unroll
-    for (int t = 0; t < 4; t++) {
-        const double u3 = u30 + t;
-        double Q = 0.0, Qz = 0.0, Qx = 0.0, Qy = 0.0;
-#pragma unroll
-        for (int kz = L; kz >= 0; kz--) {
-            if (DERIV) { Qz = Qz * u3 + Q; Qx = Qx * u3 + ax[kz]; Qy = Qy * u3 + ay[kz]; }
-            Q = Q * u3 + a[kz];
-        }
-        acc[0][t] += G[t] * Q;
-        if constexpr (DERIV != 0) {
-            const double m2Q = -2.0 * Q;
-            const double qu1 = q[0] * u1 + q[3] * u2 + q[4] * u3;
-            const double qu2 = q[3] * u1 + q[1] * u2 + q[5] * u3;
-            const double qu3 = q[4] * u1 + q[5] * u2 + q[2] * u3;
-            acc[1][t] += G[t] * (Qx + m2Q * qu1);
-            acc[2][t] += G[t] * (Qy + m2Q * qu2);
-            acc[3][t] += G[t] * (Qz + m2Q * qu3);
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------ slab form
 // A lane owns the slab of 4 x 4 grid points (rows j along n2, points t along n3) at its own n1.  The
 // polynomial is collapsed once per slab in u1 (b[ky][kz]), once per row in u2 (a[kz]) and swept by Horner
@@ -249,18 +187,13 @@ GPW_HD SlabGauss slab_gauss(const double *q, double u1, double u20, double u30) 
     }
     return G;
 }
-GPW_HD double gauss_direct(const double *q, double u1, double u2, double u3) {
-    return exp(-(q[0] * u1 * u1 + q[1] * u2 * u2 + q[2] * u3 * u3 +
-                 2.0 * (q[3] * u1 * u2 + (q[4] * u1 + q[5] * u2) * u3)));
-}
-
 // Collocation of one pair on one slab.  acc[NCOMP][16] (index j*4+t); for DERIV the gradient is
 // accumulated in grid-index (covariant) components:  d/du_i [Q G] = G (dQ/du_i + p_i Q),  p = -2 (q u).
 // ORTHO: the Gaussian along n3 relative to the row start (g3) and p_3 are the same for the four rows, p_1
 // is constant on the slab and p_2 on a row.
 template <int L, int DERIV, bool ORTHO = false>
 GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c22, double c23, double c33,
-                        double u1, double u20, double u30, double (*acc)[16]) {
+                        const SlabGauss SG, double u1, double u20, double u30, double (*acc)[16]) {
     constexpr int NB = npair2(L), NBX = npair2(L - 1);
     double b[NB], bx[NBX > 0 ? NBX : 1];
 #pragma unroll
@@ -277,7 +210,6 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
             b[bidx(L, ky, kz)] = p;
             if (DERIV && ky + kz <= L - 1) bx[bidx(L - 1, ky, kz)] = dp;
         }
-    const SlabGauss SG = slab_gauss<ORTHO>(q, u1, u20, u30);
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
     // p = -2 (q u) at the row start, its step per row and per point
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
@@ -503,86 +435,6 @@ GPW_HD double integ_expand_term(const double *B0, const double *B1, const double
     double s = kx == 0 ? B0[bidx(L, ky, kz)] : B0[bidx(L, ky, kz)] * pw1[kx];
     if (DERIV && kx > 0) s += B1[bidx(L - 1, ky, kz)] * (kx * pw1[kx - 1]);
     return s;
-}
-
-template <int L, int DERIV>
-GPW_HD void integ_slab(const double (*v)[16], const double *q, double c22, double c23, double c33, double u1,
-                       double u20, double u30, double *m) {
-    constexpr int NB = npair2(L), NBX = npair2(L - 1);
-    double B0[NB], B1[NBX > 0 ? NBX : 1];
-#pragma unroll
-    for (int i = 0; i < NB; i++) B0[i] = 0.0;
-#pragma unroll
-    for (int i = 0; i < NBX; i++) B1[i] = 0.0;
-    const SlabGauss SG = slab_gauss<false>(q, u1, u20, u30);
-    integ_slab_rows<L, DERIV, false>([&](int k, int j, double *o) {
-        for (int t = 0; t < 4; t++) o[t] = v[k][j * 4 + t];
-    }, q, c22, c23, c33, SG, u1, u20, u30, B0, B1);
-    double pw1[L + 1];
-    pw1[0] = 1.0;
-#pragma unroll
-    for (int k = 1; k <= L; k++) pw1[k] = pw1[k - 1] * u1;
-#pragma unroll
-    for (int kz = 0; kz <= L; kz++)
-#pragma unroll
-        for (int ky = 0; ky <= L - kz; ky++)
-#pragma unroll
-            for (int kx = 0; kx <= L - kz - ky; kx++)
-                m[cidx(L, kx, ky, kz)] += integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
-}
-
-// Integration of one pair on one column of four points (transpose of colloc_column).
-//   v      [NCOMP][4]: v0 and, for DERIV, the vector field already mapped to grid-index coordinates
-//   m      the thread's private moment vector (cidx order), accumulated
-template <int L, int DERIV>
-GPW_HD void integ_column(const double (*v)[4], const double *q, double cc, double u1, double u2, double u30,
-                         double *m) {
-    double G[4];
-    column_gauss(q, cc, u1, u2, u30, G);
-    double A0[L + 1], A1[L + 1], A2[L + 1], A3[L + 1];
-#pragma unroll
-    for (int kz = 0; kz <= L; kz++) { A0[kz] = 0.0; A1[kz] = 0.0; A2[kz] = 0.0; A3[kz] = 0.0; }
-#pragma unroll
-    for (int t = 0; t < 4; t++) {
-        const double u3 = u30 + t;
-        double g0 = v[0][t], g1 = 0.0, g2 = 0.0, g3 = 0.0;
-        if constexpr (DERIV != 0) {
-            const double qu1 = q[0] * u1 + q[3] * u2 + q[4] * u3;
-            const double qu2 = q[3] * u1 + q[1] * u2 + q[5] * u3;
-            const double qu3 = q[4] * u1 + q[5] * u2 + q[2] * u3;
-            g0 -= 2.0 * (v[1][t] * qu1 + v[2][t] * qu2 + v[3][t] * qu3);
-            g1 = G[t] * v[1][t]; g2 = G[t] * v[2][t]; g3 = G[t] * v[3][t];
-        }
-        g0 *= G[t];
-        double pw = 1.0;
-#pragma unroll
-        for (int kz = 0; kz <= L; kz++) {
-            A0[kz] += g0 * pw;
-            if (DERIV && kz < L) { A1[kz] += g1 * pw; A2[kz] += g2 * pw; A3[kz] += g3 * pw; }
-            pw *= u3;
-        }
-    }
-    if (DERIV) {
-#pragma unroll
-        for (int kz = 1; kz <= L; kz++) A0[kz] += kz * A3[kz - 1];
-    }
-    double p1[L + 1], p2[L + 1];
-    p1[0] = 1.0; p2[0] = 1.0;
-#pragma unroll
-    for (int k = 1; k <= L; k++) { p1[k] = p1[k - 1] * u1; p2[k] = p2[k - 1] * u2; }
-#pragma unroll
-    for (int kz = 0; kz <= L; kz++)
-#pragma unroll
-        for (int ky = 0; ky <= L - kz; ky++)
-#pragma unroll
-            for (int kx = 0; kx <= L - kz - ky; kx++) {
-                double s = A0[kz] * (p1[kx] * p2[ky]);
-                if (DERIV) {
-                    if (kx > 0) s += A1[kz] * (kx * (p1[kx - 1] * p2[ky]));
-                    if (ky > 0) s += A2[kz] * (ky * (p1[kx] * p2[ky - 1]));
-                }
-                m[cidx(L, kx, ky, kz)] += s;
-            }
 }
 
 }  // namespace gpw
