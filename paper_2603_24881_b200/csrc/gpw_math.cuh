@@ -303,13 +303,15 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
 // (contravariant) components.  vrow(comp, j, out[4]) delivers the four values of row j of component comp.
 // A lane of the integration kernel keeps B0 / B1 over ALL blocks of a brick entry: the brick is one block
 // thick along n1, so the lane's u1 is the same for every block.
-// ORTHO: the table T[kz][t] = g3(t) u3_t^kz (Gaussian along n3 relative to the row start times the power)
-// is the same for the four rows; the row's Gaussian factor multiplies the row sums instead of every point.
+// ORTHO: the Gaussian separates, G = gx(u1) gy(u2) gz(u3).  The caller passes rowg[j] = gx gy(u20 + j) and
+// g3[t] = gz(u30 + t) (SG is not used); the table T[kz][t] = g3[t] u3_t^kz is the same for the four rows and
+// the row's factor multiplies the row sums instead of every point.
 //
 // integ_expand_u1: m[cidx(L,kx,ky,kz)] (+)= B0 u1^kx + kx u1^(kx-1) B1 -- once per entry.
 template <int L, int DERIV, bool ORTHO = false, class VRow>
 GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23, double c33,
-                            const SlabGauss SG, double u1, double u20, double u30, double *B0, double *B1) {
+                            const SlabGauss SG, double u1, double u20, double u30, double *B0, double *B1,
+                            const double *rowg = nullptr, const double *g3 = nullptr) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
@@ -324,8 +326,8 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
     }
     double T[L + 1][4], p3t[4] = {0.0, 0.0, 0.0, 0.0};
     if constexpr (ORTHO) {
-        double r = SG.r3;
-        T[0][0] = 1.0; T[0][1] = r; r *= c33; T[0][2] = T[0][1] * r; r *= c33; T[0][3] = T[0][2] * r;
+#pragma unroll
+        for (int t = 0; t < 4; t++) T[0][t] = g3[t];
 #pragma unroll
         for (int kz = 1; kz <= L; kz++)
 #pragma unroll
@@ -352,18 +354,11 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
             }
 #pragma unroll
             for (int kz = 0; kz <= L; kz++) {
-                A0[kz] = kz == 0 ? fma(T[0][3], w0[3], fma(T[0][2], w0[2], fma(T[0][1], w0[1], w0[0])))
-                                 : fma(T[kz][3], w0[3], fma(T[kz][2], w0[2], fma(T[kz][1], w0[1], T[kz][0] * w0[0])));
+                A0[kz] = fma(T[kz][3], w0[3], fma(T[kz][2], w0[2], fma(T[kz][1], w0[1], T[kz][0] * w0[0])));
                 if (DERIV && kz < L) {
-                    if (kz == 0) {
-                        A1[0] = fma(T[0][3], vv[1][3], fma(T[0][2], vv[1][2], fma(T[0][1], vv[1][1], vv[1][0])));
-                        A2[0] = fma(T[0][3], vv[2][3], fma(T[0][2], vv[2][2], fma(T[0][1], vv[2][1], vv[2][0])));
-                        A3[0] = fma(T[0][3], vv[3][3], fma(T[0][2], vv[3][2], fma(T[0][1], vv[3][1], vv[3][0])));
-                    } else {
-                        A1[kz] = fma(T[kz][3], vv[1][3], fma(T[kz][2], vv[1][2], fma(T[kz][1], vv[1][1], T[kz][0] * vv[1][0])));
-                        A2[kz] = fma(T[kz][3], vv[2][3], fma(T[kz][2], vv[2][2], fma(T[kz][1], vv[2][1], T[kz][0] * vv[2][0])));
-                        A3[kz] = fma(T[kz][3], vv[3][3], fma(T[kz][2], vv[3][2], fma(T[kz][1], vv[3][1], T[kz][0] * vv[3][0])));
-                    }
+                    A1[kz] = fma(T[kz][3], vv[1][3], fma(T[kz][2], vv[1][2], fma(T[kz][1], vv[1][1], T[kz][0] * vv[1][0])));
+                    A2[kz] = fma(T[kz][3], vv[2][3], fma(T[kz][2], vv[2][2], fma(T[kz][1], vv[2][1], T[kz][0] * vv[2][0])));
+                    A3[kz] = fma(T[kz][3], vv[3][3], fma(T[kz][2], vv[3][2], fma(T[kz][1], vv[3][1], T[kz][0] * vv[3][0])));
                 }
             }
         } else {
@@ -405,7 +400,7 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
         }
         // powers of u2 (ORTHO: times the row's Gaussian factor)
         double pw2[L + 1];
-        pw2[0] = ORTHO ? grow : 1.0;
+        pw2[0] = ORTHO ? rowg[j] : 1.0;
 #pragma unroll
         for (int k = 1; k <= L; k++) pw2[k] = (k == 1 && !ORTHO) ? u2 : pw2[k - 1] * u2;
 #pragma unroll
@@ -420,8 +415,7 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
                     else B1[bidx(L - 1, ky, kz)] = fma(A1[kz], pw2[ky], B1[bidx(L - 1, ky, kz)]);
                 }
             }
-        grow *= r2; r2 *= c22;
-        if constexpr (!ORTHO) r3row *= c23;
+        if constexpr (!ORTHO) { grow *= r2; r2 *= c22; r3row *= c23; }
         if (DERIV) {
             if constexpr (ORTHO) { qr2 -= 2.0 * q[1]; }
             else { qr1 -= 2.0 * q[3]; qr2 -= 2.0 * q[1]; qr3 -= 2.0 * q[5]; }

@@ -23,7 +23,15 @@ constexpr int NGRP = 8;   // groups of 4 lanes per warp
 // padding: the four lanes of a group then read four different bank quarters with their 16-byte loads
 GPW_CX int chunk_doubles(int ncomp) { return ncomp * 16 + 2; }
 
+// ORTHO: per lane group, the 1-D Gaussian factors of the current entry along n2 and n3 over the whole brick
+// (4 BR2 + 4 BR3 values), padded so that the eight groups' 16-byte reads start in different banks
+constexpr int GT2 = 4 * BR2, GT3 = 4 * BR3;
+constexpr int GT_STRIDE = GT2 + GT3 + 2;
+static_assert(GT2 % 2 == 0 && GT3 % 2 == 0 && GT_STRIDE % 2 == 0, "16-byte alignment of the factor tables");
+
 struct BrickCtx {
+    double *gtab;            // the group's factor table (ORTHO)
+    unsigned gmask;          // the group's four lanes
     const double *vs;        // shared memory brick: chunk (block, x) at (block*4 + x) * chunk_doubles
     const double *gm;        // the level's metric (constant bank)
     int o1, o2, o3;          // stored grid index of the brick origin
@@ -48,6 +56,27 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
     const double u1 = (double)(c.o1 + c.x + en.s[0] * c.N0) - pr.nP0;
     const double u2b = (double)(c.o2 + en.s[1] * c.N1) - pr.nP1;
     const double u3b = (double)(c.o3 + en.s[2] * c.N2) - pr.nP2;
+    // ORTHO: the Gaussian separates.  Each lane fills half of one of the two 1-D tables by the recursion of
+    // Eq. (24)-(25), outwards from the table entry nearest the Gaussian's centre (so that every product is a
+    // true Gaussian value <= the start value), and evaluates the factor of its own n1 plane.
+    double gx = 1.0;
+    if constexpr (ORTHO) {
+        const int axis = c.x >> 1;
+        const int n = axis ? GT3 : GT2, lo = (c.x & 1) * (n / 2), hi = (c.x & 1) ? n : n / 2;
+        const double qa = axis ? q[2] : q[1], ua0 = axis ? u3b : u2b, ca = axis ? pr.c33 : pr.c22;
+        const int sidx = min(max(__double2int_rn(-ua0), lo), hi - 1);
+        const double us = ua0 + sidx;
+        const double gs = exp(-(qa * us * us));
+        const double rf = exp(-(qa * fma(2.0, us, 1.0))), rb = exp(qa * fma(2.0, us, -1.0));
+        double *o = c.gtab + (axis ? GT2 : 0);
+        o[sidx] = gs;
+        double gg = gs, r = rf;
+        for (int i = sidx + 1; i < hi; i++) { gg *= r; r *= ca; o[i] = gg; }
+        gg = gs; r = rb;
+        for (int i = sidx - 1; i >= lo; i--) { gg *= r; r *= ca; o[i] = gg; }
+        gx = exp(-(q[0] * u1 * u1));
+        __syncwarp();
+    }
     unsigned mask = valid ? en.mask : 0u;
     while (mask) {   // group-uniform
         const int bit = __ffs(mask) - 1;
@@ -55,14 +84,24 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
         const int t2 = bit / BR3, t3 = bit - t2 * BR3;
         const double *chunk = c.vs + (bit * 4 + c.x) * CHS;
         const double u20 = u2b + 4 * t2, u30 = u3b + 4 * t3;
-        const SlabGauss SG = slab_gauss<ORTHO>(q, u1, u20, u30);
-        integ_slab_rows<L, DERIV, ORTHO>(
-            [&](int k, int j, double *o) {
-                const double2 a = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4);
-                const double2 b = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4 + 2);
-                o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
-            },
-            q, pr.c22, pr.c23, pr.c33, SG, u1, u20, u30, B0, B1);
+        auto vrow = [&](int k, int j, double *o) {
+            const double2 a = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4);
+            const double2 b = *reinterpret_cast<const double2 *>(chunk + k * 16 + j * 4 + 2);
+            o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+        };
+        if constexpr (ORTHO) {
+            const double2 y0 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2);
+            const double2 y1 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2 + 2);
+            const double2 z0 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3);
+            const double2 z1 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2);
+            const double rowg[4] = {gx * y0.x, gx * y0.y, gx * y1.x, gx * y1.y};
+            const double g3[4] = {z0.x, z0.y, z1.x, z1.y};
+            integ_slab_rows<L, DERIV, true>(vrow, q, pr.c22, pr.c23, pr.c33, SlabGauss{0.0, 0.0, 0.0}, u1, u20, u30,
+                                            B0, B1, rowg, g3);
+        } else {
+            const SlabGauss SG = slab_gauss<false>(q, u1, u20, u30);
+            integ_slab_rows<L, DERIV, false>(vrow, q, pr.c22, pr.c23, pr.c33, SG, u1, u20, u30, B0, B1);
+        }
     }
     __syncwarp();
     // expansion in u1, sum over the group's four lanes (n1 planes), one atomic per moment
@@ -95,6 +134,7 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     constexpr int CHS = chunk_doubles(NCOMP);
     extern __shared__ __align__(16) double vs[];   // [BRICK_TILES * 4] chunks
     __shared__ unsigned s_seg[8];
+    __shared__ __align__(16) double s_gtab[ORTHO ? NWARP * NGRP * GT_STRIDE : 2];
     const BItem *itp = items + blockIdx.x;
     const int level = itp->level, brick = itp->brick;
     const unsigned it_lo = itp->lo, it_hi = itp->hi;
@@ -149,6 +189,8 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     c.o1 = 4 * BR1 * k1; c.o2 = 4 * BR2 * k2; c.o3 = 4 * BR3 * k3;
     c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
     c.x = lane & 3;
+    c.gtab = s_gtab + (ORTHO ? (warp * NGRP + grp) * GT_STRIDE : 0);
+    c.gmask = 0xfu << (4 * grp);
     const BEntry *ent = entries + ebase;
 
     // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is

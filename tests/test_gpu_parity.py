@@ -127,6 +127,12 @@ def test_config2_256_water_gga_sampled():
     _sampled_parity(inputs.make_config(2), tile_frac=0.0008, pair_frac=0.00004)
 
 
+def test_config4_512_water_gga_f_sampled():
+    """The largest instance (20480 AOs, five levels, 2.1e8 block visits) in the launch configuration
+    bench.py times."""
+    _sampled_parity(inputs.make_config(4), tile_frac=0.0005, pair_frac=0.0002)
+
+
 # ------------------------------------------------------------------------------------------ edge cases
 def test_empty_plan_and_empty_levels():
     base = inputs.make_small("cubic", deriv=1)
