@@ -303,15 +303,16 @@ GPW_HD void colloc_slab(const double *__restrict__ c, const double *q, double c2
 // (contravariant) components.  vrow(comp, j, out[4]) delivers the four values of row j of component comp.
 // A lane of the integration kernel keeps B0 / B1 over ALL blocks of a brick entry: the brick is one block
 // thick along n1, so the lane's u1 is the same for every block.
-// ORTHO: the Gaussian separates, G = gx(u1) gy(u2) gz(u3).  The caller passes rowg[j] = gx gy(u20 + j) and
-// g3[t] = gz(u30 + t) (SG is not used); the table T[kz][t] = g3[t] u3_t^kz is the same for the four rows and
-// the row's factor multiplies the row sums instead of every point.
+// ORTHO: the Gaussian separates, G = gx(u1) gy(u2) gz(u3).  The caller passes rowg[j] = gx gy(u20 + j),
+// the offsets toff[t] of the lane's four points along n3 (a permutation of 0..3: the order in which the
+// caller delivers them) and g3[t] = gz(u30 + toff[t]) (SG is not used); the table T[kz][t] = g3[t] u3_t^kz
+// is the same for the four rows and the row's factor multiplies the row sums instead of every point.
 //
 // integ_expand_u1: m[cidx(L,kx,ky,kz)] (+)= B0 u1^kx + kx u1^(kx-1) B1 -- once per entry.
 template <int L, int DERIV, bool ORTHO = false, class VRow>
 GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23, double c33,
                             const SlabGauss SG, double u1, double u20, double u30, double *B0, double *B1,
-                            const double *rowg = nullptr, const double *g3 = nullptr) {
+                            const double *rowg = nullptr, const double *g3 = nullptr, const double *toff = nullptr) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     double grow = SG.g0, r2 = SG.r2, r3row = SG.r3;
     double qr1 = 0.0, qr2 = 0.0, qr3 = 0.0;
@@ -331,10 +332,10 @@ GPW_HD void integ_slab_rows(VRow &&vrow, const double *q, double c22, double c23
 #pragma unroll
         for (int kz = 1; kz <= L; kz++)
 #pragma unroll
-            for (int t = 0; t < 4; t++) T[kz][t] = T[kz - 1][t] * (u30 + t);
+            for (int t = 0; t < 4; t++) T[kz][t] = T[kz - 1][t] * (u30 + toff[t]);
         if (DERIV) {
 #pragma unroll
-            for (int t = 0; t < 4; t++) p3t[t] = fma(-2.0 * q[2], (double)t, qr3);
+            for (int t = 0; t < 4; t++) p3t[t] = fma(-2.0 * q[2], toff[t], qr3);
         }
     }
 #pragma unroll

@@ -19,9 +19,18 @@ namespace {
 constexpr int NWARP = 4;
 constexpr int NGRP = 8;   // groups of 4 lanes per warp
 
-// shared-memory chunk = the 4 x 4 points of one n1 plane of one block, all components, plus 16 bytes of
-// padding: the four lanes of a group then read four different bank quarters with their 16-byte loads
+// Shared-memory brick, general cells: chunk = the 4 x 4 points of one n1 plane of one block, all components,
+// plus 16 bytes of padding: the four lanes of a group then read four different bank quarters with their
+// 16-byte loads.
 GPW_CX int chunk_doubles(int ncomp) { return ncomp * 16 + 2; }
+// Shared-memory brick, ORTHO: one 128-byte line per (block, component, row j) = the points t = 0,1 of the four
+// n1 planes (64 bytes, 16 banks) followed by the points t = 2,3 of the four planes (the other 16 banks).  A
+// 16-byte load instruction is served per quarter warp = two lane groups; even groups read the first half of
+// the line first and odd groups the second half (they own their four points in the order 2,3,0,1), so the two
+// groups of a quarter warp never meet in a bank, whatever blocks they are working on.
+GPW_CX int brick_doubles(int ncomp, bool ortho) {
+    return ortho ? BRICK_TILES * ncomp * 4 * 16 : BRICK_TILES * 4 * chunk_doubles(ncomp);
+}
 
 // ORTHO: per lane group, the 1-D Gaussian factors of the current entry along n2 and n3 over the whole brick
 // (4 BR2 + 4 BR3 values), padded so that the eight groups' 16-byte reads start in different banks
@@ -32,6 +41,7 @@ static_assert(GT2 % 2 == 0 && GT3 % 2 == 0 && GT_STRIDE % 2 == 0, "16-byte align
 struct BrickCtx {
     double *gtab;            // the group's factor table (ORTHO)
     unsigned gmask;          // the group's four lanes
+    int odd;                 // parity of the group within its warp
     const double *vs;        // shared memory brick: chunk (block, x) at (block*4 + x) * chunk_doubles
     const double *gm;        // the level's metric (constant bank)
     int o1, o2, o3;          // stored grid index of the brick origin
@@ -90,14 +100,24 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
             o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
         };
         if constexpr (ORTHO) {
+            const int h = c.odd;
+            const double *line = c.vs + (size_t)bit * (NCOMP * 64) + 2 * c.x;
+            auto vline = [&](int k, int j, double *o) {
+                const double *r = line + (k * 4 + j) * 16;
+                const double2 a = *reinterpret_cast<const double2 *>(r + 8 * h);
+                const double2 b = *reinterpret_cast<const double2 *>(r + 8 * (1 - h));
+                o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
+            };
             const double2 y0 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2);
             const double2 y1 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2 + 2);
-            const double2 z0 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3);
-            const double2 z1 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2);
+            const double2 z0 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2 * h);
+            const double2 z1 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2 * (1 - h));
             const double rowg[4] = {gx * y0.x, gx * y0.y, gx * y1.x, gx * y1.y};
             const double g3[4] = {z0.x, z0.y, z1.x, z1.y};
-            integ_slab_rows<L, DERIV, true>(vrow, q, pr.c22, pr.c23, pr.c33, SlabGauss{0.0, 0.0, 0.0}, u1, u20, u30,
-                                            B0, B1, rowg, g3);
+            const double t0 = (double)(2 * h), t2o = (double)(2 * (1 - h));
+            const double toff[4] = {t0, t0 + 1.0, t2o, t2o + 1.0};
+            integ_slab_rows<L, DERIV, true>(vline, q, pr.c22, pr.c23, pr.c33, SlabGauss{0.0, 0.0, 0.0}, u1, u20, u30,
+                                            B0, B1, rowg, g3, toff);
         } else {
             const SlabGauss SG = slab_gauss<false>(q, u1, u20, u30);
             integ_slab_rows<L, DERIV, false>(vrow, q, pr.c22, pr.c23, pr.c33, SG, u1, u20, u30, B0, B1);
@@ -159,6 +179,8 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
             raw[k][0] = x0.x; raw[k][1] = x0.y; raw[k][2] = x1.x; raw[k][3] = x1.y;
         }
         double *dst = vs + ((t2 * BR3 + t3) * 4 + x) * CHS + j * 4;
+        // ORTHO: line of (block, component k, row j) at ((block * NCOMP + k) * 4 + j) * 16; plane x at + 2 x, + 8 + 2 x
+        double *dsto = vs + ((size_t)(t2 * BR3 + t3) * NCOMP * 4 + j) * 16 + 2 * x;
         if constexpr (DERIV) {
             // w'_i = sum_c Hinv[i][c] w_c, so that w . grad_r f = w' . grad_u f
             double tr[4][4];
@@ -172,9 +194,17 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
             }
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                *reinterpret_cast<double2 *>(dst + k * 16) = make_double2(tr[k][0], tr[k][1]);
-                *reinterpret_cast<double2 *>(dst + k * 16 + 2) = make_double2(tr[k][2], tr[k][3]);
+                if constexpr (ORTHO) {
+                    *reinterpret_cast<double2 *>(dsto + k * 64) = make_double2(tr[k][0], tr[k][1]);
+                    *reinterpret_cast<double2 *>(dsto + k * 64 + 8) = make_double2(tr[k][2], tr[k][3]);
+                } else {
+                    *reinterpret_cast<double2 *>(dst + k * 16) = make_double2(tr[k][0], tr[k][1]);
+                    *reinterpret_cast<double2 *>(dst + k * 16 + 2) = make_double2(tr[k][2], tr[k][3]);
+                }
             }
+        } else if constexpr (ORTHO) {
+            *reinterpret_cast<double2 *>(dsto) = make_double2(raw[0][0], raw[0][1]);
+            *reinterpret_cast<double2 *>(dsto + 8) = make_double2(raw[0][2], raw[0][3]);
         } else {
             *reinterpret_cast<double2 *>(dst) = make_double2(raw[0][0], raw[0][1]);
             *reinterpret_cast<double2 *>(dst + 2) = make_double2(raw[0][2], raw[0][3]);
@@ -191,6 +221,7 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     c.x = lane & 3;
     c.gtab = s_gtab + (ORTHO ? (warp * NGRP + grp) * GT_STRIDE : 0);
     c.gmask = 0xfu << (4 * grp);
+    c.odd = grp & 1;
     const BEntry *ent = entries + ebase;
 
     // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
@@ -240,7 +271,7 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
 template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    double *mom, cudaStream_t st) {
-    constexpr int smem = BRICK_TILES * 4 * chunk_doubles(DERIV ? 4 : 1) * (int)sizeof(double);
+    constexpr int smem = brick_doubles(DERIV ? 4 : 1, ORTHO) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
         const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
