@@ -242,29 +242,44 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
             if ((cc++ % NWARP) == warp) return true;
         }
     };
-    bool have = next_chunk();
-    if (!have) return;
-    BEntry en;
-    PairRec pr;
-    en.mask = 0; en.task = 0; en.s[0] = en.s[1] = en.s[2] = 0; en.L = 0; en.pad = 0;
-    pr = PairRec{0, 0, 0, 0, 0, 0, 0, 0};
-    if (base + grp < hi) { en = ent[base + grp]; pr = load_pair(tasks, en.task); }
-    while (have) {
-        const int Lc = L;
-        const bool valid = base + grp < hi;
-        const BEntry enc = en;
-        const PairRec prc = pr;
-        have = next_chunk();
-        if (have && base + grp < hi) { en = ent[base + grp]; pr = load_pair(tasks, en.task); }   // in flight during this chunk
-        switch (Lc) {
-            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prc, valid, mom); break;
+    // Software pipeline over the warp's chunks: the entry records are loaded two chunks ahead (one 16-byte load
+    // per group), the pair records, whose address depends on the entry, one chunk ahead.
+    struct Chunk { int L; unsigned base, hi; bool ok; };
+    auto take = [&]() -> Chunk { const bool ok = next_chunk(); return Chunk{L, base, hi, ok}; };
+    const uint4 *ent4 = reinterpret_cast<const uint4 *>(ent);
+    auto load_entry = [&](const Chunk &ch) -> uint4 {
+        return (ch.ok && ch.base + grp < ch.hi) ? __ldg(ent4 + ch.base + grp) : make_uint4(0u, 0u, 0u, 0u);
+    };
+    auto decode = [](const uint4 r) -> BEntry {
+        BEntry e;
+        e.task = (int)r.x;
+        e.s[0] = (signed char)(r.y & 0xffu); e.s[1] = (signed char)((r.y >> 8) & 0xffu); e.s[2] = (signed char)((r.y >> 16) & 0xffu);
+        e.L = (unsigned char)(r.y >> 24);
+        e.mask = r.z; e.pad = r.w;
+        return e;
+    };
+    Chunk c0 = take();
+    if (!c0.ok) return;
+    Chunk c1 = take();
+    uint4 e0 = load_entry(c0), e1 = load_entry(c1);
+    PairRec p0 = load_pair(tasks, (int)e0.x);
+    while (c0.ok) {
+        const Chunk c2 = c1.ok ? take() : c1;
+        const uint4 e2 = load_entry(c2);
+        const PairRec p1 = load_pair(tasks, (int)e1.x);   // e1 was requested one chunk ago
+        const bool valid = c0.base + grp < c0.hi;
+        const BEntry enc = decode(e0);
+        switch (c0.L) {
+            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
         }
+        c0 = c1; e0 = e1; p0 = p1;
+        c1 = c2; e1 = e2;
     }
 }
 
