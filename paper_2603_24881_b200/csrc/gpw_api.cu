@@ -14,6 +14,7 @@
 #include <new>
 
 #include "gpw_kernels.cuh"
+#include "plan_device.h"
 
 namespace gpw {
 const char *last_error_cstr();
@@ -79,14 +80,8 @@ struct gpw_plan {
     // device copies
     TaskK *d_taskK = nullptr;
     TaskP *d_taskP = nullptr;
-    Visit *d_visit = nullptr;
-    Item *d_item = nullptr;
-    BEntry *d_bentry = nullptr;
-    BItem *d_bitem = nullptr;
-    long long *d_brick_base[GPW_MAX_LEVEL] = {nullptr};
+    DeviceLists lists;          // visit / brick lists and work items, built on the device (plan_device.cu)
     double *d_S = nullptr;
-    long long *d_tile_base[GPW_MAX_LEVEL] = {nullptr};
-    unsigned *d_seg[GPW_MAX_LEVEL] = {nullptr};
     double *d_coef = nullptr;   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
     double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
     double *d_vg = nullptr;     // Gaussian values of every (pair, block) visit (geometry only; written at build time)
@@ -121,20 +116,22 @@ void free_device(gpw_plan *p) {
     for (int w = 0; w < 2; w++)
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
-    cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_visit); cudaFree(p->d_item); cudaFree(p->d_S);
-    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg); cudaFree(p->d_bentry); cudaFree(p->d_bitem);
-    for (int a = 0; a < GPW_MAX_LEVEL; a++) cudaFree(p->d_brick_base[a]);
-    for (int a = 0; a < GPW_MAX_LEVEL; a++) { cudaFree(p->d_tile_base[a]); cudaFree(p->d_seg[a]); }
+    cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_S);
+    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg);
+    free_device_lists(&p->lists);
 }
 
 void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
     std::memset(&P, 0, sizeof(P));
     const HostPlan *hp = p->hp;
+    long long tile0 = 0, brick0 = 0;
     for (int a = 0; a < hp->nlevel; a++) {
         P.lev[a] = hp->lev[a];
-        P.tile_base[a] = p->d_tile_base[a];
-        P.seg[a] = p->d_seg[a];
-        P.brick_base[a] = p->d_brick_base[a];
+        // one array over all levels: the entry after a level's last block is the next level's first
+        P.tile_base[a] = p->lists.tile_base + tile0;
+        P.seg[a] = p->lists.seg + tile0 * 8;
+        P.brick_base[a] = p->lists.brick_base + brick0;
+        tile0 += hp->lev[a].ntile; brick0 += hp->lev[a].nbrick;
         P.grid[a] = grids[a];
         for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[a][L];
     }
@@ -153,15 +150,18 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     if (!plan_out) { set_error("gpw_build_pairs: plan_out is null"); return GPW_EINVAL; }
     *plan_out = nullptr;
     HostPlan *hp = nullptr;
+    int ndev = 0;
+    const bool have_dev = cudaGetDeviceCount(&ndev) == cudaSuccess && ndev >= 1;
+    if (!have_dev) cudaGetLastError();
+    // with a device the pairs are enumerated on the host and every list is built on the device; without one the
+    // host builds the lists too (introspection only: eval calls fail with GPW_ECUDA)
     const int rc = build_host_plan(cell, natm, xyz, nshl, shl_atom, shl_l, shl_nprim, shl_prim_off, prim_exp,
-                                   prim_coef, nlevel, mesh, tau, rel_cutoff, hermi, &hp);
+                                   prim_coef, nlevel, mesh, tau, rel_cutoff, hermi, !have_dev, &hp);
     if (rc != GPW_OK) return rc;
     gpw_plan *p = new (std::nothrow) gpw_plan();
     if (!p) { delete hp; set_error("out of host memory"); return GPW_ENOMEM; }
     p->hp = hp;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
-        cudaGetLastError();   // host-only plan: introspection works, eval calls fail with GPW_ECUDA
+    if (!have_dev) {   // host-only plan
         *plan_out = p;
         return GPW_OK;
     }
@@ -170,19 +170,30 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     long &nb = p->device_bytes;
     ok = ok && upload(&p->d_taskK, hp->taskK.data(), hp->taskK.size(), nb, "upload pairs");
     ok = ok && upload(&p->d_taskP, hp->taskP.data(), hp->taskP.size(), nb, "upload pairs");
-    ok = ok && upload(&p->d_visit, hp->visit.data(), hp->visit.size(), nb, "upload visit lists");
-    ok = ok && upload(&p->d_item, hp->item.data(), hp->item.size(), nb, "upload work items");
-    ok = ok && upload(&p->d_bentry, hp->bentry.data(), hp->bentry.size(), nb, "upload brick lists");
-    ok = ok && upload(&p->d_bitem, hp->bitem.data(), hp->bitem.size(), nb, "upload brick work items");
+    if (ok) {
+        const int lrc = build_device_lists(hp, &p->lists);
+        if (lrc != GPW_OK) {
+            free_device(p);
+            delete hp;
+            delete p;
+            return lrc;
+        }
+        nb += p->lists.bytes;
+        hp->nitem = p->lists.nitem; hp->nbitem = p->lists.nbitem; hp->nvisit_total = p->lists.nvisit;
+        hp->build_seconds += p->lists.seconds;
+        for (int a = 0; a < GPW_MAX_LEVEL; a++) {
+            hp->nvisit_level[a] = 0;
+            for (int i = 0; i <= MAXL; i++)
+                for (int j = 0; j <= MAXL; j++) {
+                    hp->nvisit_class[a][i][j] = (long)p->lists.cls[a][i][j];
+                    hp->nvisit_level[a] += (long)p->lists.cls[a][i][j];
+                }
+        }
+    }
     if (ok) {
         std::vector<double> S_all((size_t)hp->nlevel * S_TOTAL);
         for (int a = 0; a < hp->nlevel; a++) std::memcpy(S_all.data() + (size_t)a * S_TOTAL, hp->S[a].data(), sizeof(double) * S_TOTAL);
         ok = upload(&p->d_S, S_all.data(), S_all.size(), nb, "upload monomial maps");
-    }
-    for (int a = 0; a < hp->nlevel && ok; a++) {
-        ok = ok && upload(&p->d_tile_base[a], hp->tile_base[a].data(), hp->tile_base[a].size(), nb, "upload block offsets");
-        ok = ok && upload(&p->d_seg[a], hp->seg[a].data(), hp->seg[a].size(), nb, "upload block segments");
-        ok = ok && upload(&p->d_brick_base[a], hp->brick_base[a].data(), hp->brick_base[a].size(), nb, "upload brick offsets");
     }
     const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
     if (ok) {
@@ -199,7 +210,7 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
     if (ok) nb += (long)(sizeof(double) * nw);
     if (ok) {
-        const size_t nvg = hp->visit.size() * visit_gauss_doubles(hp->ortho);
+        const size_t nvg = (size_t)hp->nvisit_total * visit_gauss_doubles(hp->ortho);
         ok = cuda_ok(cudaMalloc((void **)&p->d_vg, sizeof(double) * (nvg ? nvg : 1)), "allocate visit Gaussians");
         if (ok) {
             nb += (long)(sizeof(double) * nvg);
@@ -208,8 +219,8 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
             fill_params(p, P, none);
             int ntile_all = 0;
             for (int a = 0; a < hp->nlevel; a++) ntile_all += hp->lev[a].ntile;
-            ok = hp->visit.empty() ||
-                 (cuda_ok(launch_visit_gauss(P, ntile_all, p->d_taskK, p->d_visit, p->d_vg, hp->ortho, 0), "visit Gaussians") &&
+            ok = hp->nvisit_total == 0 ||
+                 (cuda_ok(launch_visit_gauss(P, ntile_all, p->d_taskK, p->lists.visit, p->d_vg, hp->ortho, 0), "visit Gaussians") &&
                   cuda_ok(cudaDeviceSynchronize(), "visit Gaussians"));
         }
     }
@@ -244,7 +255,7 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
         for (int i = 0; i <= MAXL; i++)
             for (int j = 0; j <= MAXL; j++) out->nvisit_class[a][i][j] = hp->nvisit_class[a][i][j];
     }
-    out->nitem = (long)hp->item.size();
+    out->nitem = hp->nitem;
     out->ncoef_total = (long)hp->ncoef_total;
     out->build_seconds = hp->build_seconds;
     out->device_bytes = p->device_bytes + interp_bytes(p->interp);
@@ -281,7 +292,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
         const size_t nb = sizeof(double) * (size_t)g.N[0] * g.N[1] * g.N[2] * ncomp;
         if (!cuda_ok(cudaMemsetAsync(rho_dev[a], 0, nb, st), "gpw_eval_rho: memset")) return GPW_ECUDA;
     }
-    const int ntask = (int)hp->task.size(), nitem = (int)hp->item.size();
+    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return GPW_OK;
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[0][0], st); pm->ev_valid[0] = true; }
@@ -289,7 +300,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->d_visit, p->d_item, nitem, p->d_coef, p->d_vg, deriv, hp->max_L, hp->ortho, st),
+    if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef, p->d_vg, deriv, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
@@ -305,14 +316,14 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
         if (!v_dev[a]) { set_error("gpw_eval_mat: null level pointer"); return GPW_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
-    const int ntask = (int)hp->task.size(), nitem = (int)hp->item.size();
+    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return GPW_OK;
     if (!cuda_ok(cudaMemsetAsync(p->d_mom, 0, sizeof(double) * (size_t)hp->ncoef_total, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     GridParams P;
     fill_params(p, P, const_cast<double *const *>(v_dev));
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[1][0], st); pm->ev_valid[1] = true; }
-    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->d_bentry, p->d_bitem, (int)hp->bitem.size(), p->d_mom, deriv,
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_mom, deriv,
                                   hp->max_L, hp->ortho, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[1][1], st);
     DVs dv;

@@ -139,6 +139,9 @@ struct HostPlan {
     std::vector<BEntry> bentry;                      // all levels, level-major, brick-major; inside a brick by L,
                                                      // inside an L segment by decreasing number of visited blocks
     std::vector<BItem> bitem;                        // sorted by descending work
+    long nitem = 0, nbitem = 0;                      // work items of the two grid kernels
+    long long nvisit_total = 0;
+    double circ[GPW_MAX_LEVEL] = {0};                // circumradius of a 4x4x4 block about its centre, per level
     int max_L = 0;                                   // largest la + lb present
     bool ortho = false;                              // the lattice vectors are mutually orthogonal (every Gm diagonal)
     long nvisit_level[GPW_MAX_LEVEL] = {0};
@@ -161,6 +164,6 @@ void set_error(const std::string &msg);
 int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
                     const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
                     const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
-                    double tau, double rel_cutoff, int hermi, HostPlan **out);
+                    double tau, double rel_cutoff, int hermi, bool build_lists, HostPlan **out);
 
 }  // namespace gpw

@@ -143,7 +143,7 @@ void parallel_chunks(long n, long chunk, int nthread, F &&fn) {
 int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
                     const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
                     const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
-                    double tau, double rel_cutoff, int hermi, HostPlan **out) {
+                    double tau, double rel_cutoff, int hermi, bool build_lists, HostPlan **out) {
     const auto t_start = std::chrono::steady_clock::now();
     if (!cell || !xyz || !shl_atom || !shl_l || !shl_nprim || !shl_prim_off || !prim_exp || !prim_coef ||
         !mesh || !out) { set_error("gpw_build_pairs: null pointer argument"); return GPW_EINVAL; }
@@ -333,18 +333,10 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
             coff += ncoef_pad(t.la + t.lb);
             hp->ntask_level[t.level]++;
+            hp->max_L = std::max(hp->max_L, t.la + t.lb);
         }
         hp->ncoef_total = coff;
-
-        // ---- T6: blocks of every pair ----
-        std::vector<long long> lev_tile0(nlevel + 1, 0);
-        for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;
-        const long long ntile_all = lev_tile0[nlevel];
-        std::vector<long long> lev_brick0(nlevel + 1, 0);
-        for (int a = 0; a < nlevel; a++) lev_brick0[a + 1] = lev_brick0[a] + hp->lev[a].nbrick;
-        const long long nbrick_all = lev_brick0[nlevel];
         // circumradius of a block about its centre (points at +-1.5 steps per axis)
-        std::vector<double> circ(nlevel);
         for (int a = 0; a < nlevel; a++) {
             double m = 0;
             for (int sg = 0; sg < 4; sg++) {
@@ -353,8 +345,22 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                     v[x] = 1.5 * (hp->lev[a].H[x * 3 + 0] + ((sg & 1) ? -1 : 1) * hp->lev[a].H[x * 3 + 1] + ((sg & 2) ? -1 : 1) * hp->lev[a].H[x * 3 + 2]);
                 m = std::max(m, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
             }
-            circ[a] = m;
+            hp->circ[a] = m;
         }
+        if (!build_lists) {   // the block / brick lists are built on the device (plan_device.cu)
+            hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+            *out = hp;
+            return GPW_OK;
+        }
+
+        // ---- T6: blocks of every pair ----
+        std::vector<long long> lev_tile0(nlevel + 1, 0);
+        for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;
+        const long long ntile_all = lev_tile0[nlevel];
+        std::vector<long long> lev_brick0(nlevel + 1, 0);
+        for (int a = 0; a < nlevel; a++) lev_brick0[a + 1] = lev_brick0[a] + hp->lev[a].nbrick;
+        const long long nbrick_all = lev_brick0[nlevel];
+        const double *circ = hp->circ;
         const long chunk = 256;
         const long nchunk = (ntask + chunk - 1) / chunk;
         std::vector<std::vector<RawVisit>> raw(nchunk);
@@ -490,7 +496,6 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 for (const RawEntry &e : rb) {
                     BEntry &o = hp->bentry[(size_t)cur[e.key]++];
                     o.task = e.task; o.s[0] = e.s[0]; o.s[1] = e.s[1]; o.s[2] = e.s[2]; o.L = e.L; o.mask = e.mask; o.pad = 0;
-                    hp->max_L = std::max(hp->max_L, (int)e.L);
                 }
                 std::vector<RawEntry>().swap(rb);
             }
@@ -562,6 +567,9 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         }
         std::stable_sort(hp->item.begin(), hp->item.end(),
                          [](const Item &x, const Item &y) { return (x.hi - x.lo) > (y.hi - y.lo); });
+        hp->nitem = (long)hp->item.size();
+        hp->nbitem = (long)hp->bitem.size();
+        hp->nvisit_total = (long long)hp->visit.size();
     } catch (const std::bad_alloc &) {
         delete hp;
         set_error("gpw_build_pairs: out of host memory");

@@ -133,6 +133,29 @@ def test_config4_512_water_gga_f_sampled():
     _sampled_parity(inputs.make_config(4), tile_frac=0.0005, pair_frac=0.0002)
 
 
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "wrap", "contracted", "resolved"])
+def test_device_built_lists_match_oracle_visit_counts(kind):
+    """Pin G12 on the device-built lists: per (level, la, lb) the number of (pair, image, block) visits equals the
+    oracle's own enumeration (ordered pairs)."""
+    inp = inputs.make_small(kind)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp, hermi=0)
+    ocnt = o.visit_counts()
+    assert np.array_equal(plan.info["nvisit_class"], ocnt)
+    assert sum(plan.info["nvisit_level"]) == int(ocnt.sum())
+
+
+def test_device_built_lists_config1_visit_counts():
+    inp = inputs.make_config(1)
+    o = oracle.Oracle.from_inputs(inp)
+    ocnt = o.visit_counts()
+    assert np.array_equal(_plan(inp, hermi=0).info["nvisit_class"], ocnt)
+    # unordered pairs: every canonical pair but the self pairs stands for two ordered ones
+    c1 = _plan(inp, hermi=1).info["nvisit_class"]
+    self_visits = 2 * (c1 + np.transpose(c1, (0, 2, 1))) - (ocnt + np.transpose(ocnt, (0, 2, 1)))
+    assert (self_visits >= 0).all() and int(self_visits.sum()) % 2 == 0
+
+
 # ------------------------------------------------------------------------------------------ edge cases
 def test_empty_plan_and_empty_levels():
     base = inputs.make_small("cubic", deriv=1)
