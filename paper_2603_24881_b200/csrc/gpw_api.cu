@@ -30,6 +30,15 @@ __global__ void __launch_bounds__(128) k_poly_from_D(const TaskP *__restrict__ t
     pair_poly_from_D(p, D, nao, S_all + (size_t)p.level * S_TOTAL, coef + p.coef_off + 8 * (long long)t + 8);
 }
 
+// header of every pair's record in the collocation workspace (plan time)
+__global__ void __launch_bounds__(128) k_rec_headers(const TaskK *__restrict__ tk, int ntask, double *__restrict__ rec) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntask) return;
+    const TaskK k = tk[t];
+    double *h = rec + k.coef_off + 8 * (long long)t;
+    h[0] = k.nP[0]; h[1] = k.nP[1]; h[2] = k.nP[2]; h[3] = k.ap; h[4] = k.c22; h[5] = k.c23; h[6] = k.c33; h[7] = 0.0;
+}
+
 struct DVs { double v[GPW_MAX_LEVEL]; };
 
 __global__ void __launch_bounds__(128) k_F_from_moments(const TaskP *__restrict__ tp, int ntask,
@@ -197,15 +206,16 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     }
     const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
     if (ok) {
-        // collocation records: [nP0 nP1 nP2 a_p c22 c23 c33 c11 | polynomial] per pair, headers written once
-        std::vector<double> rec(nw + 8 * hp->taskK.size(), 0.0);
-        for (size_t i = 0; i < hp->taskK.size(); i++) {
-            const TaskK &k = hp->taskK[i];
-            double *h = rec.data() + k.coef_off + 8 * (long long)i;
-            h[0] = k.nP[0]; h[1] = k.nP[1]; h[2] = k.nP[2]; h[3] = k.ap; h[4] = k.c22; h[5] = k.c23; h[6] = k.c33;
-            h[7] = std::exp(-2.0 * k.ap * hp->lev[hp->task[i].level].Gm[0]);
+        // collocation records: [nP0 nP1 nP2 a_p c22 c23 c33 0 | polynomial] per pair, headers written once
+        const size_t nrec = nw + 8 * hp->taskK.size();
+        ok = cuda_ok(cudaMalloc((void **)&p->d_coef, sizeof(double) * nrec), "allocate pair records") &&
+             cuda_ok(cudaMemsetAsync(p->d_coef, 0, sizeof(double) * nrec, 0), "clear pair records");
+        if (ok) {
+            nb += (long)(sizeof(double) * nrec);
+            const int nt = (int)hp->taskK.size();
+            if (nt) k_rec_headers<<<(nt + 127) / 128, 128>>>(p->d_taskK, nt, p->d_coef);
+            ok = cuda_ok(cudaGetLastError(), "pair record headers");
         }
-        ok = upload(&p->d_coef, rec.data(), rec.size(), nb, "upload pair records");
     }
     ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
     if (ok) nb += (long)(sizeof(double) * nw);

@@ -32,7 +32,7 @@ __device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, in
 }
 
 // launchers (each picks the instantiation for the plan's largest L; ortho: every level's Gm is diagonal)
-// rec: per-pair records of the collocation kernel, header (8 doubles: nP[3], a_p, c22, c23, c33, c11) followed
+// rec: per-pair records of the collocation kernel, header (8 doubles: nP[3], a_p, c22, c23, c33, 0) followed
 // by the pair polynomial; the record of pair i of class (level, L) starts at coef_base[level][L] + i * (8 + ncoef_pad(L))
 // vg: Gaussian values of every visit (visit_gauss_doubles(ortho) per visit, order of `visits`), written once per
 // plan by launch_visit_gauss

@@ -300,41 +300,71 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         size_t nt = 0;
         for (auto &v : per_shell) nt += v.size();
         if (nt > 2000000000ull) { delete hp; set_error("gpw_build_pairs: more than 2^31 pairs"); return GPW_EUNSUPPORTED; }
-        hp->task.reserve(nt);
-        for (auto &v : per_shell) { hp->task.insert(hp->task.end(), v.begin(), v.end()); std::vector<HostTask>().swap(v); }
-        // sort by (level, L), keeping enumeration order inside a group
-        std::stable_sort(hp->task.begin(), hp->task.end(), [](const HostTask &x, const HostTask &y) {
-            if (x.level != y.level) return x.level < y.level;
-            return (x.la + x.lb) < (y.la + y.lb);
+        // counting sort by class (level, L), keeping enumeration order inside a class: per shell the number of
+        // its pairs in every class, prefix sums over (class, shell), then every shell scatters its own pairs
+        constexpr int NCLS = GPW_MAX_LEVEL * 8;
+        auto cls_of = [](const HostTask &t) { return t.level * 8 + t.la + t.lb; };
+        std::vector<long> start((size_t)nshl * NCLS, 0);
+        parallel_chunks(nshl, 16, nthread, [&](long, long lo, long hi, int) {
+            for (long sa = lo; sa < hi; sa++)
+                for (const HostTask &t : per_shell[sa]) start[(size_t)sa * NCLS + cls_of(t)]++;
+        });
+        long cls_first[NCLS + 1];
+        {
+            long run = 0;
+            for (int c = 0; c < NCLS; c++) {
+                cls_first[c] = run;
+                for (long sa = 0; sa < nshl; sa++) {
+                    const long n = start[(size_t)sa * NCLS + c];
+                    start[(size_t)sa * NCLS + c] = run;
+                    run += n;
+                }
+            }
+            cls_first[NCLS] = run;
+        }
+        hp->task.resize(nt);
+        parallel_chunks(nshl, 16, nthread, [&](long, long lo, long hi, int) {
+            for (long sa = lo; sa < hi; sa++) {
+                long *pos = &start[(size_t)sa * NCLS];
+                for (const HostTask &t : per_shell[sa]) hp->task[(size_t)pos[cls_of(t)]++] = t;
+                std::vector<HostTask>().swap(per_shell[sa]);
+            }
         });
         const long ntask = (long)hp->task.size();
         hp->taskK.resize(ntask); hp->taskP.resize(ntask);
+        // inside a class the workspace offset is affine in the pair index: coef_base + i * ncoef_pad(L)
         long long coff = 0;
-        for (long i = 0; i < ntask; i++) {
-            const HostTask &t = hp->task[i];
-            const LevelGeom &g = hp->lev[t.level];
-            TaskK &k = hp->taskK[i];
-            for (int a = 0; a < 3; a++)
-                k.nP[a] = (t.P[0] * hp->binv[0 * 3 + a] + t.P[1] * hp->binv[1 * 3 + a] + t.P[2] * hp->binv[2 * 3 + a]) * g.N[a];
-            k.ap = t.ap;
-            k.c22 = std::exp(-2.0 * t.ap * g.Gm[1]);
-            k.c23 = std::exp(-2.0 * t.ap * g.Gm[5]);
-            k.c33 = std::exp(-2.0 * t.ap * g.Gm[2]);
-            k.coef_off = coff;
-            TaskP &p = hp->taskP[i];
-            for (int x = 0; x < 3; x++) { p.PA[x] = t.P[x] - t.A[x]; p.PB[x] = t.P[x] - t.Bt[x]; }
-            p.pref = t.pref; p.coef_off = coff;
-            p.ao_a = hp->ao_loc[t.shl_a]; p.ao_b = hp->ao_loc[t.shl_b];
-            p.la = (short)t.la; p.lb = (short)t.lb; p.level = (short)t.level; p.sym = (short)t.sym;
-            // pairs are sorted by (level, L): inside a class the workspace offset is affine in the pair index
-            if (!hp->coef_base_set[t.level][t.la + t.lb]) {
-                hp->coef_base_set[t.level][t.la + t.lb] = true;
-                hp->coef_base[t.level][t.la + t.lb] = coff - (long long)i * ncoef_pad(t.la + t.lb);
-            }
-            coff += ncoef_pad(t.la + t.lb);
-            hp->ntask_level[t.level]++;
-            hp->max_L = std::max(hp->max_L, t.la + t.lb);
+        for (int c = 0; c < NCLS; c++) {
+            const long n = cls_first[c + 1] - cls_first[c];
+            const int level = c / 8, L = c % 8;
+            if (n == 0 || L > MAXLP) continue;
+            hp->coef_base_set[level][L] = true;
+            hp->coef_base[level][L] = coff - (long long)cls_first[c] * ncoef_pad(L);
+            coff += (long long)n * ncoef_pad(L);
+            hp->ntask_level[level] += n;
+            hp->max_L = std::max(hp->max_L, L);
         }
+        parallel_chunks(ntask, 4096, nthread, [&](long, long lo, long hi, int) {
+            for (long i = lo; i < hi; i++) {
+                const HostTask &t = hp->task[i];
+                const LevelGeom &g = hp->lev[t.level];
+                const int L = t.la + t.lb;
+                const long long off = hp->coef_base[t.level][L] + (long long)i * ncoef_pad(L);
+                TaskK &k = hp->taskK[i];
+                for (int a = 0; a < 3; a++)
+                    k.nP[a] = (t.P[0] * hp->binv[0 * 3 + a] + t.P[1] * hp->binv[1 * 3 + a] + t.P[2] * hp->binv[2 * 3 + a]) * g.N[a];
+                k.ap = t.ap;
+                k.c22 = std::exp(-2.0 * t.ap * g.Gm[1]);
+                k.c23 = std::exp(-2.0 * t.ap * g.Gm[5]);
+                k.c33 = std::exp(-2.0 * t.ap * g.Gm[2]);
+                k.coef_off = off;
+                TaskP &p = hp->taskP[i];
+                for (int x = 0; x < 3; x++) { p.PA[x] = t.P[x] - t.A[x]; p.PB[x] = t.P[x] - t.Bt[x]; }
+                p.pref = t.pref; p.coef_off = off;
+                p.ao_a = hp->ao_loc[t.shl_a]; p.ao_b = hp->ao_loc[t.shl_b];
+                p.la = (short)t.la; p.lb = (short)t.lb; p.level = (short)t.level; p.sym = (short)t.sym;
+            }
+        });
         hp->ncoef_total = coff;
         // circumradius of a block about its centre (points at +-1.5 steps per axis)
         for (int a = 0; a < nlevel; a++) {
