@@ -82,6 +82,25 @@ def model_flops_from_counts(counts, deriv: int) -> float:
     return tot
 
 
+def rank_seed(config: int, rank: int):
+    """Seed of rank's workload: rank 0 takes the config's own seed, every other rank an independent workload
+    of the same shape (weak scaling, no data-path collective)."""
+    from paper_2603_24881_b200 import inputs
+    return None if rank == 0 else inputs.BASE_SEED + config + 1000 * rank
+
+
+def reduce_over_ranks(ms_step: float, flops_step: float, dist, device):
+    """Whole-job figures: the slowest rank's time per step and the flops of all ranks."""
+    if dist is None:
+        return ms_step, flops_step
+    import torch
+    t = torch.tensor([ms_step], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    f = torch.tensor([flops_step], dtype=torch.float64, device=device)
+    dist.all_reduce(f, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(f.item())
+
+
 def time_oracle_sample(inp, budget_s: float = 20.0):
     """The oracle as it stands on a bounded, seeded sample of the workload: all visits of a random set
     of 4x4x4 blocks (eval_rho) and of a random set of shell pairs (eval_mat).  Returns (GFLOP/s in the
@@ -170,7 +189,7 @@ def main():
     W = max(3, args.warmup)
 
     # every rank its own independent workload of the same shape (weak scaling)
-    inp = inputs.make_config(args.config, seed=inputs.BASE_SEED + args.config + 1000 * rank if rank else None)
+    inp = inputs.make_config(args.config, seed=rank_seed(args.config, rank))
     deriv, nc = inp.deriv, inp.ncomp
     t0 = time.time()
     plan = gpw.gpw_build_pairs(*inp.abi_args())
@@ -228,15 +247,7 @@ def main():
     sampler.stop()
     kt /= args.steps
     ms_step = ms_total / args.steps
-    if dist is not None:
-        t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
-        f = torch.tensor([flops_step], dtype=torch.float64, device="cuda")
-        dist.all_reduce(f, op=dist.ReduceOp.SUM)
-        flops_all = float(f.item())
-    else:
-        flops_all = flops_step
+    ms_step, flops_all = reduce_over_ranks(ms_step, flops_step, dist, "cuda")
     value = flops_all / (ms_step * 1e-3) / 1e9
 
     # parity-side sanity on the very buffers that were timed: adjointness <rho[D], v> dV = Tr(D F[v])
@@ -297,10 +308,7 @@ def main():
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1) / e2e_steps
-    if dist is not None:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms, _ = reduce_over_ranks(e2e_ms, flops_step, dist, "cuda")
     e2e_value = flops_all / (e2e_ms * 1e-3) / 1e9
 
     if rank != 0:
