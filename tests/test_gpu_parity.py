@@ -215,3 +215,34 @@ def test_repeat_calls_overwrite_outputs():
     assert relmax(r2[0], 2.0 * r1[0]) <= 1e-13
     v = [inp.v(0)]
     assert relmax(gpu_mat(plan, v, 0), gpu_mat(plan, v, 0)) <= 1e-13
+
+
+def test_eval_on_a_side_stream_and_two_plans_interleaved():
+    """The eval calls are asynchronous on the caller's stream and keep no state between plans: two plans
+    used alternately on a non-default stream give the same results as each alone on the default stream."""
+    import torch
+    a = inputs.make_small("cubic", deriv=1)
+    b = inputs.make_small("triclinic", deriv=1)
+    pa, pb = _plan(a), _plan(b)
+    ref = {}
+    for name, inp, plan in (("a", a, pa), ("b", b, pb)):
+        v = [inp.v(l) for l in range(inp.nlevel)]
+        ref[name] = (gpu_rho(plan, inp.D(), 1), gpu_mat(plan, v, 1))
+    side = torch.cuda.Stream()
+    out = {}
+    with torch.cuda.stream(side):
+        for rep in range(2):
+            for name, inp, plan in (("a", a, pa), ("b", b, pb)):
+                D = torch.as_tensor(inp.D(), device="cuda")
+                rho = [torch.full((4,) + tuple(int(x) for x in m), float("nan"), dtype=torch.float64, device="cuda") for m in plan.mesh]
+                vd = [torch.as_tensor(inp.v(l), device="cuda") for l in range(inp.nlevel)]
+                F = torch.full((plan.nao, plan.nao), float("nan"), dtype=torch.float64, device="cuda")
+                gpw.gpw_eval_rho(plan, D, 1, rho)
+                gpw.gpw_eval_mat(plan, vd, 1, F)
+                out[name] = (rho, F)
+    side.synchronize()
+    for name in ("a", "b"):
+        rho, F = out[name]
+        for got, want in zip(rho, ref[name][0]):
+            assert relmax(got.cpu().numpy(), want) <= 1e-13
+        assert relmax(F.cpu().numpy(), ref[name][1]) <= 1e-13
