@@ -15,6 +15,8 @@
 // to shared memory once, so that no prefetched value waits in registers (the accumulators take 128 of the
 // 255 registers of the GGA variant; a bulk-copy version was measured slower: cp.async.bulk is a
 // warp-uniform instruction, eight different sources per chunk serialise).
+#include <type_traits>
+
 #include "gpw_kernels.cuh"
 
 namespace gpw {
@@ -92,7 +94,8 @@ __device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, un
 }
 
 template <int L, int LMAX, int DERIV, bool ORTHO>
-__device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long vi, const double *s, double (*acc)[16]) {
+__device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long vi, const double *s, bool valid,
+                                             double (*acc)[16]) {
     const double ap = s[3];
     double q[6];
 #pragma unroll
@@ -102,7 +105,7 @@ __device__ __forceinline__ void colloc_visit(const ColCtx &c, unsigned long long
     const double u30 = (double)(c.n3 + visit_wrap(vi, 2) * c.N2) - s[2];
     const double *gv = s + slot_vg(LMAX);
     SlabGauss SG;
-    SG.g0 = gv[c.x];
+    SG.g0 = valid ? gv[c.x] : 0.0;   // a group without a visit of its own adds zeros (see the chunk loop)
     SG.r2 = ORTHO ? gv[4] : gv[4 + c.x];
     SG.r3 = ORTHO ? gv[5] : gv[8 + c.x];
     colloc_slab<L, DERIV, ORTHO>(s + 8, q, s[4], s[5], s[6], SG, u1, u20, u30, acc);
@@ -159,17 +162,20 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
     // ---- chunk table: entry = (first visit relative to it.lo, L | visits << 8) ----
     const unsigned myseg = P.seg[it.level][(size_t)it.tile * 8 + (lane & 7)];
     int nch = 0;
-#pragma unroll 1
+    int kend[LMAX + 1];      // one past the last chunk of every L segment
+#pragma unroll
     for (int L = 0; L <= LMAX; L++) {
         const unsigned lo = max(it.lo, __shfl_sync(0xffffffffu, myseg, L));
         const unsigned hi = min(it.hi, __shfl_sync(0xffffffffu, myseg, L + 1));
-        if (lo >= hi) continue;
-        const int n = (int)((hi - lo + NGRP - 1) / NGRP);
-        for (int k = lane; k < n; k += 32) {
-            const unsigned base = lo + NGRP * k;
-            if (nch + k < MAXCH) tab[nch + k] = make_uint2(base - it.lo, (unsigned)L | (min(hi - base, (unsigned)NGRP) << 8));
+        if (lo < hi) {
+            const int n = (int)((hi - lo + NGRP - 1) / NGRP);
+            for (int k = lane; k < n; k += 32) {
+                const unsigned base = lo + NGRP * k;
+                if (nch + k < MAXCH) tab[nch + k] = make_uint2(base - it.lo, (unsigned)L | (min(hi - base, (unsigned)NGRP) << 8));
+            }
+            nch += n;
         }
-        nch += n;
+        kend[L] = min(nch, MAXCH);
     }
     nch = min(nch, MAXCH);   // cannot bind: at most MAXVIS / NGRP full chunks + one ragged chunk per L segment
 
@@ -208,27 +214,58 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
     };
     stage_chunk(0, 0);
     stage_chunk(1, 1);
-    int slot = 0;
+    // One loop per L segment, its body straight-line code: a group without a visit of its own in a ragged chunk
+    // evaluates group 0's visit with a zero Gaussian instead of branching around the evaluation, so that the
+    // control work of the next chunks (table and visit records, cp.async addresses) can be scheduled into the
+    // FP64 instruction stream.
+    int slot = 0, k = 0;
+    auto run_segment = [&](auto Lc, int k_end) {
+        constexpr int L = decltype(Lc)::value;
 #pragma unroll 1
-    for (int k = 0; k < nch; k++) {
-        cp_async_wait<1>();   // chunk k has landed (chunk k+1 may still be in flight)
-        __syncwarp();         // ... for all four lanes of the group; and every lane has left the slot refilled next
-        stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
-        const uint2 e = tab[k];
-        if ((unsigned)grp < (e.y >> 8)) {
-            const unsigned long long v0 = vis[e.x + grp];
-            const double *s = c.slot + slot * SLOT;
-            switch ((int)(e.y & 0xffu)) {
-                case 0: colloc_visit<0, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 1: colloc_visit<1, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 2: colloc_visit<2, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 3: if constexpr (LMAX >= 3) colloc_visit<3, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 4: if constexpr (LMAX >= 4) colloc_visit<4, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                case 5: if constexpr (LMAX >= 5) colloc_visit<5, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-                default: if constexpr (LMAX >= 6) colloc_visit<6, LMAX, DERIV, ORTHO>(c, v0, s, acc); break;
-            }
+        for (; k < k_end; k++) {
+            cp_async_wait<1>();   // chunk k has landed (chunk k+1 may still be in flight)
+            __syncwarp();         // ... for all four lanes of the group; and every lane has left the slot refilled next
+            stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
+            const uint2 e = tab[k];
+            const bool valid = (unsigned)grp < (e.y >> 8);
+            const int gi = valid ? grp : 0;
+            const unsigned long long v0 = vis[e.x + gi];
+            colloc_visit<L, LMAX, DERIV, ORTHO>(c, v0, wsm + (size_t)gi * GSTRIDE + slot * SLOT, valid, acc);
+            if (++slot == NSLOT) slot = 0;
         }
-        if (++slot == NSLOT) slot = 0;
+    };
+    if constexpr (LMAX <= 4 || DERIV == 0) {
+        run_segment(std::integral_constant<int, 0>{}, kend[0]);
+        run_segment(std::integral_constant<int, 1>{}, kend[1]);
+        run_segment(std::integral_constant<int, 2>{}, kend[2]);
+        if constexpr (LMAX >= 3) run_segment(std::integral_constant<int, 3>{}, kend[3]);
+        if constexpr (LMAX >= 4) run_segment(std::integral_constant<int, 4>{}, kend[4]);
+        if constexpr (LMAX >= 5) run_segment(std::integral_constant<int, 5>{}, kend[5]);
+        if constexpr (LMAX >= 6) run_segment(std::integral_constant<int, 6>{}, kend[6]);
+    } else {
+        // deriv = 1 with f shells (L up to 6): the straight-line form costs registers the L = 5, 6 bodies do not
+        // have (measured on cfg 4: 7 % slower); one loop, the evaluation behind a branch
+#pragma unroll 1
+        for (; k < nch; k++) {
+            cp_async_wait<1>();
+            __syncwarp();
+            stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
+            const uint2 e = tab[k];
+            if ((unsigned)grp < (e.y >> 8)) {
+                const unsigned long long v0 = vis[e.x + grp];
+                const double *s = c.slot + slot * SLOT;
+                switch ((int)(e.y & 0xffu)) {
+                    case 0: colloc_visit<0, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 1: colloc_visit<1, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 2: colloc_visit<2, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 3: colloc_visit<3, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 4: colloc_visit<4, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 5: colloc_visit<5, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    default: colloc_visit<6, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                }
+            }
+            if (++slot == NSLOT) slot = 0;
+        }
     }
     cp_async_wait<0>();
     __syncwarp();
