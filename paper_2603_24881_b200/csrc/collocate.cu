@@ -204,12 +204,12 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 
     // ---- software pipeline over the chunks: the records of chunk k+2 are in flight while chunk k is evaluated;
     //      one commit group per chunk (empty past the end), so "all but the newest" = chunks <= k complete ----
+    // Branch-free: past the last chunk the last one is staged again (into a slot nobody reads any more), and a
+    // group without a visit of its own copies group 0's record into its own slot.
     auto stage_chunk = [&](int k, int slot) {
-        if (k < nch) {
-            const uint2 e = tab[k];
-            if ((unsigned)grp < (e.y >> 8))
-                stage_visit<LMAX, ORTHO>(c, (int)(e.y & 0xffu), visit_task(vis[e.x + grp]), e.x + grp, c.slot + slot * SLOT);
-        }
+        const uint2 e = tab[min(k, nch - 1)];
+        const unsigned iv = e.x + ((unsigned)grp < (e.y >> 8) ? grp : 0);
+        stage_visit<LMAX, ORTHO>(c, (int)(e.y & 0xffu), visit_task(vis[iv]), iv, c.slot + slot * SLOT);
         cp_async_commit();
     };
     stage_chunk(0, 0);
