@@ -1,6 +1,6 @@
 // Collocation kernel (Eq. 3; the work of Alg. 1, re-decomposed for B200).
 //
-// One warp per work item = one 4x4x4 grid block and a range of its visit list.  The warp is eight groups
+// One warp (= one CTA) per work item = one 4x4x4 grid block and a range of its visit list: eight groups
 // of four lanes; a group evaluates one (pair, block) visit at a time and a lane owns the slab of 4x4 grid
 // points at its own n1, so the polynomial collapse in u1 and the Gaussian set-up are paid once per 16
 // points (gpw_math.cuh, colloc_slab).  Every lane keeps its rho values (and, for DERIV, the gradient in
@@ -23,7 +23,10 @@ namespace gpw {
 namespace {
 
 constexpr int NGRP = 8;     // groups of 4 lanes per warp
-constexpr int NWARP = 4;    // warps (work items) per CTA
+// warps (work items) per CTA.  One: a warp's registers and shared memory go to the next item the moment it
+// finishes, instead of waiting for the slowest of four items (measured: cfg2 k_collocate 3.58 -> 3.47 ms,
+// cfg4 30.8 -> 29.6 ms; two warps per CTA: no gain)
+constexpr int NWARP = 1;
 constexpr int NSLOT = 3;    // shared-memory slots per group (copy issued two chunks ahead)
 constexpr int MAXCH = 64;   // chunks per item: ITEM_MAX / NGRP full ones + one ragged chunk per L segment
 constexpr int MAXVIS = 384; // visits per item (ITEM_MAX of plan.cpp)
@@ -56,17 +59,6 @@ struct ColCtx {
     int N0, N1, N2;
     int x;                 // lane within the group
 };
-
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(unsigned smem, const void *gmem) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async8(unsigned smem, const void *gmem) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // A visit record is its raw 8 bytes: task in the low word, the three signed wrap counts in bytes 4..6.
 __device__ __forceinline__ int visit_task(unsigned long long r) { return (int)(unsigned)r; }
@@ -133,7 +125,7 @@ __device__ __forceinline__ int group_reduce_scatter(double *a, int lane) {
 }
 
 template <int DERIV, int LMAX, bool ORTHO>
-__global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_constant__ GridParams P,
+__global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_collocate(const __grid_constant__ GridParams P,
                                                                    const Visit *__restrict__ visits,
                                                                    const Item *__restrict__ items, int nitem,
                                                                    const double *__restrict__ rec,
@@ -154,7 +146,7 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 
     // ---- the item's visit records -> shared memory (first cp.async group) ----
     {
-        const Visit *src = visits + P.tile_base[it.level][it.tile] + it.lo;
+        const Visit *src = visits + it.vstart;
         const int n = min((int)(it.hi - it.lo), MAXVIS);   // cannot bind: items have at most MAXVIS visits
         for (int i = lane; i < n; i += 32) cp_async8(smem_u32(vis + i), src + i);
         cp_async_commit();
@@ -181,7 +173,7 @@ __global__ void __launch_bounds__(128, DERIV ? 2 : 3) k_collocate(const __grid_c
 
     ColCtx c;
     c.rec = rec;
-    c.vg = vg + (size_t)(P.tile_base[it.level][it.tile] + it.lo) * vg_doubles(ORTHO);
+    c.vg = vg + (size_t)it.vstart * vg_doubles(ORTHO);
     c.gm = g.Gm;
     c.coef_base = P.coef_base[it.level];
     c.slot = wsm + (size_t)grp * GSTRIDE;

@@ -83,7 +83,10 @@ struct Item {
     unsigned lo, hi;      // visit range relative to the block's list
     int single;           // 1: the only item of its block (plain store), 0: accumulate atomically
     int pad;
+    long long vstart;     // index of the item's first visit in the plan's visit list (= tile_base of the block + lo):
+                          // saves the collocation warp one dependent load at its start
 };
+static_assert(sizeof(Item) == 32, "Item must be 32 bytes");
 
 // One (pair, lattice image, brick) entry of a brick's list: which of the brick's blocks the pair visits.
 struct BEntry {

@@ -31,6 +31,18 @@ __device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, in
     return r;
 }
 
+// cp.async helpers (records staged in shared memory ahead of their use)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(unsigned smem, const void *gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async8(unsigned smem, const void *gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // launchers (each picks the instantiation for the plan's largest L; ortho: every level's Gm is diagonal)
 // rec: per-pair records of the collocation kernel, header (8 doubles: nP[3], a_p, c22, c23, c33, 0) followed
 // by the pair polynomial; the record of pair i of class (level, L) starts at coef_base[level][L] + i * (8 + ncoef_pad(L))

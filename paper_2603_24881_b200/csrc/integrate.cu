@@ -50,8 +50,13 @@ struct BrickCtx {
 };
 
 template <int L, int DERIV, bool ORTHO>
-__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const PairRec pr, bool valid,
+__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const double *prs, bool valid,
                                             double *__restrict__ mom) {
+    // the pair record (TaskK) staged in the group's shared-memory slot
+    PairRec pr;
+    pr.nP0 = prs[0]; pr.nP1 = prs[1]; pr.nP2 = prs[2]; pr.ap = prs[3];
+    pr.c22 = prs[4]; pr.c23 = prs[5]; pr.c33 = prs[6];
+    pr.coef_off = __double_as_longlong(prs[7]);
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int CHS = chunk_doubles(NCOMP);
     constexpr int NB = npair2(L), NBX = npair2(L - 1);
@@ -155,11 +160,55 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     extern __shared__ __align__(16) double vs[];   // [BRICK_TILES * 4] chunks
     __shared__ unsigned s_seg[8];
     __shared__ __align__(16) double s_gtab[ORTHO ? NWARP * NGRP * GT_STRIDE : 2];
+    __shared__ __align__(16) double s_pair[NWARP * NGRP * 2 * 8];   // per group: two slots of one pair record
     const BItem *itp = items + blockIdx.x;
     const int level = itp->level, brick = itp->brick;
     const unsigned it_lo = itp->lo, it_hi = itp->hi;
     const long long ebase = itp->base;
     if (threadIdx.x < 8) s_seg[threadIdx.x] = itp->seg[threadIdx.x];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane >> 2;
+    const BEntry *ent = entries + ebase;
+    __syncthreads();   // s_seg
+
+    // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
+    // warp-uniform); the chunks are dealt to the CTA's warps round robin.
+    int L = -1, cc = 0;
+    unsigned base = 0, hi = 0;
+    auto next_chunk = [&]() -> bool {
+        for (;;) {
+            base += NGRP;
+            if (L < 0 || base >= hi) {
+                do {
+                    L++;
+                    if (L > LMAX) return false;
+                    base = max(it_lo, s_seg[L]);
+                    hi = min(it_hi, s_seg[L + 1]);
+                } while (base >= hi);
+            }
+            if ((cc++ % NWARP) == warp) return true;
+        }
+    };
+    // Software pipeline over the warp's chunks: the entry records are loaded two chunks ahead (one 16-byte load
+    // per group), the pair records, whose address depends on the entry, one chunk ahead.
+    struct Chunk { int L; unsigned base, hi; bool ok; };
+    auto take = [&]() -> Chunk { const bool ok = next_chunk(); return Chunk{L, base, hi, ok}; };
+    const uint4 *ent4 = reinterpret_cast<const uint4 *>(ent);
+    auto load_entry = [&](const Chunk &ch) -> uint4 {
+        return (ch.ok && ch.base + grp < ch.hi) ? __ldg(ent4 + ch.base + grp) : make_uint4(0u, 0u, 0u, 0u);
+    };
+    auto decode = [](const uint4 r) -> BEntry {
+        BEntry e;
+        e.task = (int)r.x;
+        e.s[0] = (signed char)(r.y & 0xffu); e.s[1] = (signed char)((r.y >> 8) & 0xffu); e.s[2] = (signed char)((r.y >> 16) & 0xffu);
+        e.L = (unsigned char)(r.y >> 24);
+        e.mask = r.z; e.pad = r.w;
+        return e;
+    };
+    // the first two chunks' entry records are in flight while the brick is staged
+    Chunk c0 = take();
+    Chunk c1 = take();
+    uint4 e0 = load_entry(c0), e1 = load_entry(c1);
+
     const LevelGeom &g = P.lev[level];
     const int B2 = g.B[2], B1n = g.B[1];
     const int k3 = brick % B2, k2 = (brick / B2) % B1n, k1 = brick / (B2 * B1n);
@@ -210,9 +259,18 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
             *reinterpret_cast<double2 *>(dst + 2) = make_double2(raw[0][2], raw[0][3]);
         }
     }
+    // Pair records (TaskK, 64 bytes) reach the group's shared-memory slot by cp.async, 16 bytes per lane, one chunk
+    // ahead of their use (a record prefetched into registers was spilled to the stack at once, which made the
+    // warp wait for the load: 6 % of the warp samples of profile r01g)
+    double *mypair = s_pair + (warp * NGRP + grp) * 16;
+    auto stage_pair = [&](unsigned task, int slot) {
+        cp_async16(smem_u32(mypair + slot * 8) + 16 * (lane & 3), reinterpret_cast<const char *>(tasks + task) + 16 * (lane & 3));
+        cp_async_commit();
+    };
+    stage_pair(e0.x, 0);
     __syncthreads();
+    if (!c0.ok) { cp_async_wait<0>(); return; }
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane >> 2;
     BrickCtx c;
     c.vs = vs;
     c.gm = g.Gm;
@@ -222,65 +280,32 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     c.gtab = s_gtab + (ORTHO ? (warp * NGRP + grp) * GT_STRIDE : 0);
     c.gmask = 0xfu << (4 * grp);
     c.odd = grp & 1;
-    const BEntry *ent = entries + ebase;
 
-    // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
-    // warp-uniform); the chunks are dealt to the CTA's warps round robin.
-    int L = -1, cc = 0;
-    unsigned base = 0, hi = 0;
-    auto next_chunk = [&]() -> bool {
-        for (;;) {
-            base += NGRP;
-            if (L < 0 || base >= hi) {
-                do {
-                    L++;
-                    if (L > LMAX) return false;
-                    base = max(it_lo, s_seg[L]);
-                    hi = min(it_hi, s_seg[L + 1]);
-                } while (base >= hi);
-            }
-            if ((cc++ % NWARP) == warp) return true;
-        }
-    };
-    // Software pipeline over the warp's chunks: the entry records are loaded two chunks ahead (one 16-byte load
-    // per group), the pair records, whose address depends on the entry, one chunk ahead.
-    struct Chunk { int L; unsigned base, hi; bool ok; };
-    auto take = [&]() -> Chunk { const bool ok = next_chunk(); return Chunk{L, base, hi, ok}; };
-    const uint4 *ent4 = reinterpret_cast<const uint4 *>(ent);
-    auto load_entry = [&](const Chunk &ch) -> uint4 {
-        return (ch.ok && ch.base + grp < ch.hi) ? __ldg(ent4 + ch.base + grp) : make_uint4(0u, 0u, 0u, 0u);
-    };
-    auto decode = [](const uint4 r) -> BEntry {
-        BEntry e;
-        e.task = (int)r.x;
-        e.s[0] = (signed char)(r.y & 0xffu); e.s[1] = (signed char)((r.y >> 8) & 0xffu); e.s[2] = (signed char)((r.y >> 16) & 0xffu);
-        e.L = (unsigned char)(r.y >> 24);
-        e.mask = r.z; e.pad = r.w;
-        return e;
-    };
-    Chunk c0 = take();
-    if (!c0.ok) return;
-    Chunk c1 = take();
-    uint4 e0 = load_entry(c0), e1 = load_entry(c1);
-    PairRec p0 = load_pair(tasks, (int)e0.x);
+    int ps = 0;
     while (c0.ok) {
         const Chunk c2 = c1.ok ? take() : c1;
         const uint4 e2 = load_entry(c2);
-        const PairRec p1 = load_pair(tasks, (int)e1.x);   // e1 was requested one chunk ago
+        __syncwarp();                 // every lane has left the slot refilled next
+        stage_pair(e1.x, ps ^ 1);     // e1 was requested one chunk ago
+        cp_async_wait<1>();           // this chunk's record has landed
+        __syncwarp();                 // ... for all four lanes of the group
+        const double *prs = mypair + ps * 8;
         const bool valid = c0.base + grp < c0.hi;
         const BEntry enc = decode(e0);
         switch (c0.L) {
-            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, p0, valid, mom); break;
+            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
         }
-        c0 = c1; e0 = e1; p0 = p1;
+        c0 = c1; e0 = e1;
         c1 = c2; e1 = e2;
+        ps ^= 1;
     }
+    cp_async_wait<0>();
 }
 
 template <int DERIV, int LMAX, bool ORTHO>

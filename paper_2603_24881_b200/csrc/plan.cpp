@@ -591,6 +591,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                     it.lo = (unsigned)((unsigned long long)n * p / nparts);
                     it.hi = (unsigned)((unsigned long long)n * (p + 1) / nparts);
                     it.single = nparts == 1; it.pad = 0;
+                    it.vstart = hp->tile_base[a][tl] + it.lo;
                     hp->item.push_back(it);
                 }
             }

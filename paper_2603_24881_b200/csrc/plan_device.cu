@@ -203,6 +203,7 @@ __global__ void k_items_fill(const __grid_constant__ ListGeom G, const long long
         it.lo = (unsigned)((unsigned long long)n * p / np);
         it.hi = (unsigned)((unsigned long long)n * (p + 1) / np);
         it.single = np == 1; it.pad = 0;
+        it.vstart = base[b] + it.lo;
         items[off[b] + p] = it;
         key[off[b] + p] = ITEM_MAX - (it.hi - it.lo);   // ascending key = decreasing length
     }
