@@ -211,6 +211,11 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     // control work of the next chunks (table and visit records, cp.async addresses) can be scheduled into the
     // FP64 instruction stream.
     int slot = 0, k = 0;
+    // the chunk's table entry and the group's visit record are read one chunk ahead (they are in shared memory
+    // from the start), which takes two dependent shared-memory loads off the head of every chunk
+    bool valid = (unsigned)grp < (tab[0].y >> 8);
+    int gi = valid ? grp : 0;
+    unsigned long long v0 = vis[tab[0].x + gi];
     auto run_segment = [&](auto Lc, int k_end) {
         constexpr int L = decltype(Lc)::value;
 #pragma unroll 1
@@ -218,11 +223,12 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
             cp_async_wait<1>();   // chunk k has landed (chunk k+1 may still be in flight)
             __syncwarp();         // ... for all four lanes of the group; and every lane has left the slot refilled next
             stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
-            const uint2 e = tab[k];
-            const bool valid = (unsigned)grp < (e.y >> 8);
-            const int gi = valid ? grp : 0;
-            const unsigned long long v0 = vis[e.x + gi];
+            const uint2 en = tab[min(k + 1, nch - 1)];
+            const bool valid_n = (unsigned)grp < (en.y >> 8);
+            const int gi_n = valid_n ? grp : 0;
+            const unsigned long long v_n = vis[en.x + gi_n];
             colloc_visit<L, LMAX, DERIV, ORTHO>(c, v0, wsm + (size_t)gi * GSTRIDE + slot * SLOT, valid, acc);
+            valid = valid_n; gi = gi_n; v0 = v_n;
             if (++slot == NSLOT) slot = 0;
         }
     };
@@ -261,32 +267,34 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     }
     cp_async_wait<0>();
     __syncwarp();
-    // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i (linear: before the sum)
+    // The eight groups worked on different visits of the same block: sum every component's 16 slab values over
+    // the groups; afterwards the lane holds the two points off, off + 1 of its slab (same row), all components.
+    int off = 0;
+#pragma unroll
+    for (int k = 0; k < NCOMP; k++) off = group_reduce_scatter<16>(acc[k], lane);
+    // gradient: grid-index components -> Cartesian, d/dX_c = sum_i Hinv[i][c] d/du_i -- after the sum, on the
+    // lane's two points instead of the sixteen of the slab
     if constexpr (DERIV != 0) {
 #pragma unroll
-        for (int i = 0; i < 16; i++) {
+        for (int i = 0; i < 2; i++) {
             const double d1 = acc[1][i], d2 = acc[2][i], d3 = acc[3][i];
 #pragma unroll
             for (int k = 0; k < 3; k++)
                 acc[1 + k][i] = g.Hinv[0 * 3 + k] * d1 + g.Hinv[1 * 3 + k] * d2 + g.Hinv[2 * 3 + k] * d3;
         }
     }
-    // the eight groups worked on different visits of the same block
-    double *flat = &acc[0][0];
-    const int off = group_reduce_scatter<NCOMP * 16>(flat, lane);
     const size_t ng = (size_t)g.N[0] * g.N[1] * g.N[2];
-    constexpr int PER = NCOMP * 16 / 8;            // 8 (two rows of one component) or 2 (half a row)
-    const int comp = off >> 4, j = (off & 15) >> 2, t0 = off & 3;
-    double *out = P.grid[it.level] + comp * ng + ((size_t)c.n1 * g.N[1] + c.n2 + j) * g.N[2] + c.n3 + t0;
+    const int j = off >> 2, t0 = off & 3;
+    double *out = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2 + j) * g.N[2] + c.n3 + t0;
     if (it.single) {
 #pragma unroll
-        for (int i = 0; i < PER; i += 2) {
-            double *o = out + (i >> 2) * g.N[2] + (i & 3);
-            *reinterpret_cast<double2 *>(o) = make_double2(flat[i], flat[i + 1]);
-        }
+        for (int k = 0; k < NCOMP; k++) *reinterpret_cast<double2 *>(out + k * ng) = make_double2(acc[k][0], acc[k][1]);
     } else {
 #pragma unroll
-        for (int i = 0; i < PER; i++) atomicAdd(out + (i >> 2) * g.N[2] + (i & 3), flat[i]);
+        for (int k = 0; k < NCOMP; k++) {
+            atomicAdd(out + k * ng, acc[k][0]);
+            atomicAdd(out + k * ng + 1, acc[k][1]);
+        }
     }
 }
 
