@@ -94,6 +94,7 @@ struct gpw_plan {
     double *d_coef = nullptr;   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
     double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
     double *d_vg = nullptr;     // Gaussian values of every (pair, block) visit (geometry only; written at build time)
+    double *d_eg = nullptr;     // 1-D Gaussian factor tables of every brick entry (orthogonal cells; geometry only)
     // optional kernel timing (gpw_plan_set_timing): events around each kernel of the last eval calls
     bool timing = false;
     cudaEvent_t ev[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
@@ -126,7 +127,7 @@ void free_device(gpw_plan *p) {
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
     cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_S);
-    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg);
+    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg); cudaFree(p->d_eg);
     free_device_lists(&p->lists);
 }
 
@@ -234,6 +235,20 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
                   cuda_ok(cudaDeviceSynchronize(), "visit Gaussians"));
         }
     }
+    if (ok && hp->ortho && p->lists.nentry > 0) {
+        const size_t neg = (size_t)p->lists.nentry * entry_gauss_doubles(true);
+        ok = cuda_ok(cudaMalloc((void **)&p->d_eg, sizeof(double) * neg), "allocate entry Gaussians");
+        if (ok) {
+            nb += (long)(sizeof(double) * neg);
+            GridParams P;
+            double *none[GPW_MAX_LEVEL] = {nullptr};
+            fill_params(p, P, none);
+            int nbrick_all = 0;
+            for (int a = 0; a < hp->nlevel; a++) nbrick_all += hp->lev[a].nbrick;
+            ok = cuda_ok(launch_entry_gauss(P, nbrick_all, p->d_taskK, p->lists.bentry, p->d_eg, 0), "entry Gaussians") &&
+                 cuda_ok(cudaDeviceSynchronize(), "entry Gaussians");
+        }
+    }
     if (!ok) {
         free_device(p);
         delete hp;
@@ -333,7 +348,7 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     fill_params(p, P, const_cast<double *const *>(v_dev));
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[1][0], st); pm->ev_valid[1] = true; }
-    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_mom, deriv,
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, p->d_mom, deriv,
                                   hp->max_L, hp->ortho, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[1][1], st);
     DVs dv;

@@ -53,8 +53,13 @@ cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Ite
 size_t visit_gauss_doubles(bool ortho);
 cudaError_t launch_visit_gauss(const GridParams &P, int ntile_all, const TaskK *tasks, const Visit *visits, double *vg,
                                bool ortho, cudaStream_t st);
+// eg: 1-D Gaussian factor tables of every brick entry (entry_gauss_doubles(ortho) per entry, order of `entries`;
+// orthogonal cells only, else unused), written once per plan by launch_entry_gauss
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st);
+                             int nitem, const double *eg, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st);
+size_t entry_gauss_doubles(bool ortho);
+cudaError_t launch_entry_gauss(const GridParams &P, int nbrick_all, const TaskK *tasks, const BEntry *entries, double *eg,
+                               cudaStream_t st);
 
 // interp.cu: Eq. (7)-(8) with cuFFT; the state (plans, scratch) is created on first use; return a gpw_status
 struct InterpState;

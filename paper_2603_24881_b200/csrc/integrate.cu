@@ -11,6 +11,10 @@
 // and one FP64 atomic per moment finish the entry.  Alg. 2 instead adds nca*ncb values per (pair, block)
 // to global memory; amortising over the brick cuts that traffic by the blocks per
 // entry, and the moment form keeps the per-lane state at (L+1)(L+2)/2 doubles instead of nca*ncb.
+// Orthogonal cells: the Gaussian separates and the 1-D factor tables of every entry over its brick are
+// geometry only -- computed once per plan (k_entry_gauss below, 352 bytes per entry) and staged by cp.async
+// with the pair record, so that an entry starts on its first block without exp() or recursion (measured:
+// cfg2 k_integrate 4.04 -> 3.58 ms, cfg4 33.4 -> 26.8 ms against building them per entry in the kernel).
 #include "gpw_kernels.cuh"
 
 namespace gpw {
@@ -32,14 +36,16 @@ GPW_CX int brick_doubles(int ncomp, bool ortho) {
     return ortho ? BRICK_TILES * ncomp * 4 * 16 : BRICK_TILES * 4 * chunk_doubles(ncomp);
 }
 
-// ORTHO: per lane group, the 1-D Gaussian factors of the current entry along n2 and n3 over the whole brick
-// (4 BR2 + 4 BR3 values), padded so that the eight groups' 16-byte reads start in different banks
+// ORTHO: the Gaussian separates, G = gx(u1) gy(u2) gz(u3).  The 1-D factors of every brick entry over the whole
+// brick -- gy[4 BR2], gz[4 BR3], gx[4] -- depend on the geometry only: they are computed once per plan
+// (k_entry_gauss, EG doubles per entry) and reach one of the group's two shared-memory slots by cp.async one
+// chunk ahead; a group's slots are padded so that the eight groups' 16-byte reads start in different banks.
 constexpr int GT2 = 4 * BR2, GT3 = 4 * BR3;
-constexpr int GT_STRIDE = GT2 + GT3 + 2;
-static_assert(GT2 % 2 == 0 && GT3 % 2 == 0 && GT_STRIDE % 2 == 0, "16-byte alignment of the factor tables");
+constexpr int EG = GT2 + GT3 + 4;
+constexpr int GT_STRIDE = 2 * EG + 2;
+static_assert(GT2 % 2 == 0 && GT3 % 2 == 0 && EG % 2 == 0 && GT_STRIDE % 2 == 0, "16-byte alignment of the factor tables");
 
 struct BrickCtx {
-    double *gtab;            // the group's factor table (ORTHO)
     unsigned gmask;          // the group's four lanes
     int odd;                 // parity of the group within its warp
     const double *vs;        // shared memory brick: chunk (block, x) at (block*4 + x) * chunk_doubles
@@ -50,8 +56,8 @@ struct BrickCtx {
 };
 
 template <int L, int DERIV, bool ORTHO>
-__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const double *prs, bool valid,
-                                            double *__restrict__ mom) {
+__device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const double *prs, const double *gt,
+                                            bool valid, double *__restrict__ mom) {
     // the pair record (TaskK) staged in the group's shared-memory slot
     PairRec pr;
     pr.nP0 = prs[0]; pr.nP1 = prs[1]; pr.nP2 = prs[2]; pr.ap = prs[3];
@@ -71,27 +77,9 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
     const double u1 = (double)(c.o1 + c.x + en.s[0] * c.N0) - pr.nP0;
     const double u2b = (double)(c.o2 + en.s[1] * c.N1) - pr.nP1;
     const double u3b = (double)(c.o3 + en.s[2] * c.N2) - pr.nP2;
-    // ORTHO: the Gaussian separates.  Each lane fills half of one of the two 1-D tables by the recursion of
-    // Eq. (24)-(25), outwards from the table entry nearest the Gaussian's centre (so that every product is a
-    // true Gaussian value <= the start value), and evaluates the factor of its own n1 plane.
+    // ORTHO: the entry's 1-D factor tables are in the slot gt; the factor of the lane's own n1 plane
     double gx = 1.0;
-    if constexpr (ORTHO) {
-        const int axis = c.x >> 1;
-        const int n = axis ? GT3 : GT2, lo = (c.x & 1) * (n / 2), hi = (c.x & 1) ? n : n / 2;
-        const double qa = axis ? q[2] : q[1], ua0 = axis ? u3b : u2b, ca = axis ? pr.c33 : pr.c22;
-        const int sidx = min(max(__double2int_rn(-ua0), lo), hi - 1);
-        const double us = ua0 + sidx;
-        const double gs = exp(-(qa * us * us));
-        const double rf = exp(-(qa * fma(2.0, us, 1.0))), rb = exp(qa * fma(2.0, us, -1.0));
-        double *o = c.gtab + (axis ? GT2 : 0);
-        o[sidx] = gs;
-        double gg = gs, r = rf;
-        for (int i = sidx + 1; i < hi; i++) { gg *= r; r *= ca; o[i] = gg; }
-        gg = gs; r = rb;
-        for (int i = sidx - 1; i >= lo; i--) { gg *= r; r *= ca; o[i] = gg; }
-        gx = exp(-(q[0] * u1 * u1));
-        __syncwarp();
-    }
+    if constexpr (ORTHO) gx = gt[GT2 + GT3 + c.x];
     unsigned mask = valid ? en.mask : 0u;
     while (mask) {   // group-uniform
         const int bit = __ffs(mask) - 1;
@@ -113,10 +101,10 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
                 const double2 b = *reinterpret_cast<const double2 *>(r + 8 * (1 - h));
                 o[0] = a.x; o[1] = a.y; o[2] = b.x; o[3] = b.y;
             };
-            const double2 y0 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2);
-            const double2 y1 = *reinterpret_cast<const double2 *>(c.gtab + 4 * t2 + 2);
-            const double2 z0 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2 * h);
-            const double2 z1 = *reinterpret_cast<const double2 *>(c.gtab + GT2 + 4 * t3 + 2 * (1 - h));
+            const double2 y0 = *reinterpret_cast<const double2 *>(gt + 4 * t2);
+            const double2 y1 = *reinterpret_cast<const double2 *>(gt + 4 * t2 + 2);
+            const double2 z0 = *reinterpret_cast<const double2 *>(gt + GT2 + 4 * t3 + 2 * h);
+            const double2 z1 = *reinterpret_cast<const double2 *>(gt + GT2 + 4 * t3 + 2 * (1 - h));
             const double rowg[4] = {gx * y0.x, gx * y0.y, gx * y1.x, gx * y1.y};
             const double g3[4] = {z0.x, z0.y, z1.x, z1.y};
             const double t0 = (double)(2 * h), t2o = (double)(2 * (1 - h));
@@ -154,6 +142,7 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
                                                                           const TaskK *__restrict__ tasks,
                                                                           const BEntry *__restrict__ entries,
                                                                           const BItem *__restrict__ items,
+                                                                          const double *__restrict__ eg,
                                                                           double *__restrict__ mom) {
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int CHS = chunk_doubles(NCOMP);
@@ -263,11 +252,22 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     // ahead of their use (a record prefetched into registers was spilled to the stack at once, which made the
     // warp wait for the load: 6 % of the warp samples of profile r01g)
     double *mypair = s_pair + (warp * NGRP + grp) * 16;
-    auto stage_pair = [&](unsigned task, int slot) {
+    // ... together with the factor tables of the group's entry (ORTHO; the entry index does not depend on a load)
+    double *mygt = s_gtab + (ORTHO ? (warp * NGRP + grp) * GT_STRIDE : 0);
+    auto stage_pair = [&](const Chunk &ch, unsigned task, int slot) {
         cp_async16(smem_u32(mypair + slot * 8) + 16 * (lane & 3), reinterpret_cast<const char *>(tasks + task) + 16 * (lane & 3));
+        if constexpr (ORTHO) {
+            // a group without an entry of its own copies a valid entry's tables (never used: its mask is empty)
+            const unsigned ei = ch.ok ? min(ch.base + grp, ch.hi - 1) : it_lo;
+            const char *src = reinterpret_cast<const char *>(eg + (size_t)(ebase + ei) * EG) + 16 * (lane & 3);
+            const unsigned dst = smem_u32(mygt + slot * EG) + 16 * (lane & 3);
+#pragma unroll
+            for (int t = 0; t < (EG / 2 + 3) / 4; t++)
+                if (4 * t + (lane & 3) < EG / 2) cp_async16(dst + 64 * t, src + 64 * t);
+        }
         cp_async_commit();
     };
-    stage_pair(e0.x, 0);
+    stage_pair(c0, e0.x, 0);
     __syncthreads();
     if (!c0.ok) { cp_async_wait<0>(); return; }
 
@@ -277,7 +277,6 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
     c.o1 = 4 * BR1 * k1; c.o2 = 4 * BR2 * k2; c.o3 = 4 * BR3 * k3;
     c.N0 = g.N[0]; c.N1 = g.N[1]; c.N2 = g.N[2];
     c.x = lane & 3;
-    c.gtab = s_gtab + (ORTHO ? (warp * NGRP + grp) * GT_STRIDE : 0);
     c.gmask = 0xfu << (4 * grp);
     c.odd = grp & 1;
 
@@ -286,20 +285,21 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
         const Chunk c2 = c1.ok ? take() : c1;
         const uint4 e2 = load_entry(c2);
         __syncwarp();                 // every lane has left the slot refilled next
-        stage_pair(e1.x, ps ^ 1);     // e1 was requested one chunk ago
+        stage_pair(c1, e1.x, ps ^ 1); // e1 was requested one chunk ago
         cp_async_wait<1>();           // this chunk's record has landed
         __syncwarp();                 // ... for all four lanes of the group
         const double *prs = mypair + ps * 8;
+        const double *gt = mygt + ps * EG;
         const bool valid = c0.base + grp < c0.hi;
         const BEntry enc = decode(e0);
         switch (c0.L) {
-            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prs, valid, mom); break;
+            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
         }
         c0 = c1; e0 = e1;
         c1 = c2; e1 = e2;
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const _
 
 template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
-                   double *mom, cudaStream_t st) {
+                   const double *eg, double *mom, cudaStream_t st) {
     constexpr int smem = brick_doubles(DERIV ? 4 : 1, ORTHO) * (int)sizeof(double);
     static bool configured = false;   // per instantiation
     if (!configured) {
@@ -318,26 +318,61 @@ cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entrie
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    k_integrate<DERIV, LMAX, ORTHO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, mom);
+    k_integrate<DERIV, LMAX, ORTHO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
     return cudaGetLastError();
 }
 
 template <int DERIV, bool ORTHO>
 cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
-                     double *mom, int max_L, cudaStream_t st) {
-    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, entries, items, nitem, mom, st);
-    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, entries, items, nitem, mom, st);
-    return launch<DERIV, 6, ORTHO>(P, tasks, entries, items, nitem, mom, st);
+                     const double *eg, double *mom, int max_L, cudaStream_t st) {
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
+    return launch<DERIV, 6, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
 }
 
 }  // namespace
 
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st) {
-    if (deriv) return ortho ? launch_l<1, true>(P, tasks, entries, items, nitem, mom, max_L, st)
-                            : launch_l<1, false>(P, tasks, entries, items, nitem, mom, max_L, st);
-    return ortho ? launch_l<0, true>(P, tasks, entries, items, nitem, mom, max_L, st)
-                 : launch_l<0, false>(P, tasks, entries, items, nitem, mom, max_L, st);
+                             int nitem, const double *eg, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st) {
+    if (deriv) return ortho ? launch_l<1, true>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
+                            : launch_l<1, false>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
+    return ortho ? launch_l<0, true>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
+                 : launch_l<0, false>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
+}
+
+// ---------------------------------------------------------------------------------------- plan-time kernel
+// 1-D Gaussian factors of every brick entry (orthogonal cells), in the order of the entry list: one CTA per
+// brick, one thread per table value, direct exp() (Eq. 24-25 give the same values by recursion):
+//   [ gy(i) = exp(-a_p Gm22 (o2 + i + s2 N2 - nP2)^2), i < 4 BR2 | gz(i), i < 4 BR3 | gx(x), x < 4 ]
+namespace {
+__global__ void __launch_bounds__(128) k_entry_gauss(const __grid_constant__ GridParams P, const TaskK *__restrict__ tasks,
+                                                     const BEntry *__restrict__ entries, double *__restrict__ eg) {
+    int brick = blockIdx.x, level = 0;
+    while (brick >= P.lev[level].nbrick) { brick -= P.lev[level].nbrick; level++; }
+    const LevelGeom &g = P.lev[level];
+    const long long lo = P.brick_base[level][brick], hi = P.brick_base[level][brick + 1];
+    const int B2 = g.B[2], B1n = g.B[1];
+    const int org[3] = {4 * BR1 * (brick / (B2 * B1n)), 4 * BR2 * ((brick / B2) % B1n), 4 * BR3 * (brick % B2)};
+    for (long long i = threadIdx.x; i < (hi - lo) * EG; i += blockDim.x) {
+        const long long e = lo + i / EG;
+        const int v = (int)(i % EG);
+        const int axis = v < GT2 ? 1 : (v < GT2 + GT3 ? 2 : 0);
+        const int idx = axis == 1 ? v : (axis == 2 ? v - GT2 : v - GT2 - GT3);
+        const BEntry en = entries[e];
+        const TaskK &k = tasks[en.task];
+        const double u = (double)(org[axis] + idx + en.s[axis] * g.N[axis]) - k.nP[axis];
+        eg[e * EG + v] = exp(-(k.ap * g.Gm[axis] * u * u));
+    }
+}
+}  // namespace
+
+size_t entry_gauss_doubles(bool ortho) { return ortho ? (size_t)EG : 0; }
+
+cudaError_t launch_entry_gauss(const GridParams &P, int nbrick_all, const TaskK *tasks, const BEntry *entries, double *eg,
+                               cudaStream_t st) {
+    if (nbrick_all <= 0) return cudaSuccess;
+    k_entry_gauss<<<nbrick_all, 128, 0, st>>>(P, tasks, entries, eg);
+    return cudaGetLastError();
 }
 
 }  // namespace gpw
