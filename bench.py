@@ -362,7 +362,7 @@ def main():
         "fock_build_ms": fock_ms,
         "fock_build_note": "eval_rho + gpw_interp_up + gpw_restrict_down of a synthetic fine-grid N(0,1) field + eval_mat; "
                            "XC and Hartree excluded",
-        "plan_build_s": build_s,
+        "plan_build_s": build_s, "plan_device_bytes": int(info["device_bytes"]),
         "adjointness_rel_err": adj,
     }
     if not args.no_cpu_baseline:
