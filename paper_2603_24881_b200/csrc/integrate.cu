@@ -138,7 +138,9 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
 }
 
 template <int DERIV, int LMAX, bool ORTHO>
-__global__ void __launch_bounds__(NWARP * 32, DERIV ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
+// deriv = 0 with f shells (L up to 6): three CTAs per SM leave 168 registers and the L = 5, 6 bodies spill; two CTAs
+// at 220 registers without spills are faster (cfg3 k_integrate 2.40 -> 2.31 ms)
+__global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX > 4) ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
                                                                           const TaskK *__restrict__ tasks,
                                                                           const BEntry *__restrict__ entries,
                                                                           const BItem *__restrict__ items,
