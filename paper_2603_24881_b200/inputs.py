@@ -265,6 +265,7 @@ def make_small(kind: str, seed: int = 1, deriv: int = 0, tau: float = 1e-10,
       'cubic'      2 atoms (s,p,d | s,p), cubic 7 Bohr, one 28^3 mesh
       'triclinic'  2 atoms (s,p,d,f | s,p,d), sheared cell, meshes 36x32x28 and 20x16x16
       'wrap'       1+1 atoms with diffuse shells in a 5 Bohr cell (R_t > cell edge), 16^3
+      'ortho'      2 atoms, s..f / s..d, orthorhombic 6 x 7.5 x 9 Bohr, meshes 24x36x44, 12x20x24
       'contracted' 2 atoms, shells with 3 primitives each, cubic 8 Bohr, meshes 32^3, 16^3
       'resolved'   2 atoms, soft exponents on a fine mesh (a_p h^2 <= 0.3) for
                    quadrature-exact checks (v = 1 -> overlap; electron count)
@@ -283,6 +284,14 @@ def make_small(kind: str, seed: int = 1, deriv: int = 0, tau: float = 1e-10,
         shells = [_single_prim_shells([0, 1, 2, 3], _loguniform(rng, 0.25, 2.5, 4)),
                   _single_prim_shells([0, 1, 2], _loguniform(rng, 0.25, 2.5, 3))]
         mesh = [[36, 32, 28], [20, 16, 16]]
+    elif kind == "ortho":
+        # orthorhombic, three different edges and meshes (ragged bricks along n2 and n3): the separable-Gaussian
+        # path with a different metric, mesh and brick count per axis
+        cell = np.diag([6.0, 7.5, 9.0])
+        xyz = np.array([[1.1, 6.9, 2.0], [3.6, 3.0, 8.4]])
+        shells = [_single_prim_shells([0, 1, 2, 3], _loguniform(rng, 0.25, 2.5, 4)),
+                  _single_prim_shells([0, 1, 2], _loguniform(rng, 0.25, 2.5, 3))]
+        mesh = [[24, 36, 44], [12, 20, 24]]
     elif kind == "wrap":
         cell = np.eye(3) * 5.0
         xyz = np.array([[0.7, 4.4, 2.5], [-0.9, 1.0, 6.1]])

@@ -51,7 +51,7 @@ def test_argument_validation():
     expect(binding.GPW_EINVAL, 14, 2)                                     # hermi
 
 
-@pytest.mark.parametrize("kind", ["triclinic", "wrap", "contracted"])
+@pytest.mark.parametrize("kind", ["triclinic", "ortho", "wrap", "contracted"])
 def test_plan_matches_oracle_enumeration(kind):
     inp = inputs.make_small(kind)
     o = oracle.Oracle.from_inputs(inp)

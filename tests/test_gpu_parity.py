@@ -25,7 +25,7 @@ def _plan(inp, hermi=None):
     return p
 
 
-@pytest.mark.parametrize("kind", ["cubic", "triclinic", "wrap", "contracted", "resolved"])
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "ortho", "wrap", "contracted", "resolved"])
 @pytest.mark.parametrize("deriv", [0, 1])
 @pytest.mark.parametrize("hermi", [1, 0])
 def test_small_cells_full_parity(kind, deriv, hermi):
@@ -133,7 +133,7 @@ def test_config4_512_water_gga_f_sampled():
     _sampled_parity(inputs.make_config(4), tile_frac=0.0005, pair_frac=0.0002)
 
 
-@pytest.mark.parametrize("kind", ["cubic", "triclinic", "wrap", "contracted", "resolved"])
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "ortho", "wrap", "contracted", "resolved"])
 def test_device_built_lists_match_oracle_visit_counts(kind):
     """Pin G12 on the device-built lists: per (level, la, lb) the number of (pair, image, block) visits equals the
     oracle's own enumeration (ordered pairs)."""

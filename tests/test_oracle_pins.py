@@ -148,7 +148,7 @@ def test_task_set_levels_and_tiles_by_brute_force():
 
 
 # ---------------------------------------------------------------- G1/G2: against the plain definition
-@pytest.mark.parametrize("kind,deriv", [("cubic", 1), ("triclinic", 0), ("wrap", 1), ("contracted", 0)])
+@pytest.mark.parametrize("kind,deriv", [("cubic", 1), ("triclinic", 0), ("ortho", 0), ("wrap", 1), ("contracted", 0)])
 def test_truncated_matches_plain_definition(kind, deriv):
     """north_star: untruncated brute force over all lattice images on tiny cells, rel 1e-8 at tau = 1e-10."""
     inp = inputs.make_small(kind, deriv=deriv)
