@@ -26,7 +26,11 @@ namespace gpw {
 namespace {
 
 constexpr unsigned ITEM_MAX = 384;    // visits per collocation work item
-constexpr unsigned BITEM_MAX = 768;   // entries per integration work item
+// entries per integration work item: an item stages its brick of v once, so longer items stage less (cfg2 / cfg4
+// k_integrate -2 % with 1536), but only while enough items are left to balance the SMs (cfg3: +3 %); the longer
+// form is used when it still leaves BITEM_PER_SM items per SM
+constexpr unsigned BITEM_MAX = 768, BITEM_BIG = 1536;
+constexpr long long BITEM_PER_SM = 40;
 
 __device__ __forceinline__ int floordiv_d(int n, int d) { return n >= 0 ? n / d : -((-n + d - 1) / d); }
 __device__ __forceinline__ int posmod_d(int n, int d) { const int m = n % d; return m < 0 ? m + d : m; }
@@ -461,10 +465,16 @@ int build_device_lists(const HostPlan *hp, DeviceLists *out) {
             long long *ioff = nullptr;
             BItem *it = nullptr, *it2 = nullptr;
             GPW_ALLOC(&np, (size_t)nbrick_all, "brick items"); GPW_ALLOC(&ioff, (size_t)nbrick_all, "brick items");
-            k_items_count<<<(unsigned)((nbrick_all + 255) / 256), 256, 0, st>>>(out->brick_base, nbrick_all, np, BITEM_MAX);
-            GPW_TRY(cudaGetLastError(), "brick items");
+            int dev = 0, nsm = 0;
+            GPW_TRY(cudaGetDevice(&dev), "brick items");
+            GPW_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "brick items");
             long long nbitem = 0;
-            if ((rc = scan_counts(S, np, nbrick_all, ioff, &nbitem, st)) != GPW_OK) return rc;
+            for (unsigned maxlen : {BITEM_BIG, BITEM_MAX}) {
+                k_items_count<<<(unsigned)((nbrick_all + 255) / 256), 256, 0, st>>>(out->brick_base, nbrick_all, np, maxlen);
+                GPW_TRY(cudaGetLastError(), "brick items");
+                if ((rc = scan_counts(S, np, nbrick_all, ioff, &nbitem, st)) != GPW_OK) return rc;
+                if (nbitem >= BITEM_PER_SM * nsm) break;
+            }
             GPW_ALLOC(&ikey, (size_t)nbitem, "brick items"); GPW_ALLOC(&ikey2, (size_t)nbitem, "brick items");
             GPW_ALLOC(&it, (size_t)nbitem, "brick items");
             if (!S.alloc(&it2, (size_t)nbitem, &nb)) return fail("brick items", cudaErrorMemoryAllocation);
