@@ -26,10 +26,11 @@ namespace gpw {
 namespace {
 
 constexpr unsigned ITEM_MAX = 384;    // visits per collocation work item
-// entries per integration work item: an item stages its brick of v once, so longer items stage less (cfg2 / cfg4
-// k_integrate -2 % with 1536), but only while enough items are left to balance the SMs (cfg3: +3 %); the longer
-// form is used when it still leaves BITEM_PER_SM items per SM
-constexpr unsigned BITEM_MAX = 768, BITEM_BIG = 1536;
+// entries per integration work item: an item stages its brick of v once, so longer items stage less (cfg2
+// k_integrate 3.58 -> 3.51 -> 3.46 ms, cfg4 26.8 -> 26.1 -> 25.3 ms with 768 -> 1536 -> 3072), but only while enough
+// items are left to balance the SMs (cfg3: +3 % with 1536; cfg4: +3 % with one item per brick); the longest form that
+// still leaves BITEM_PER_SM items per SM is used
+constexpr unsigned BITEM_MAX = 768, BITEM_BIG = 1536, BITEM_HUGE = 3072;
 constexpr long long BITEM_PER_SM = 40;
 
 __device__ __forceinline__ int floordiv_d(int n, int d) { return n >= 0 ? n / d : -((-n + d - 1) / d); }
@@ -469,7 +470,7 @@ int build_device_lists(const HostPlan *hp, DeviceLists *out) {
             GPW_TRY(cudaGetDevice(&dev), "brick items");
             GPW_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "brick items");
             long long nbitem = 0;
-            for (unsigned maxlen : {BITEM_BIG, BITEM_MAX}) {
+            for (unsigned maxlen : {BITEM_HUGE, BITEM_BIG, BITEM_MAX}) {
                 k_items_count<<<(unsigned)((nbrick_all + 255) / 256), 256, 0, st>>>(out->brick_base, nbrick_all, np, maxlen);
                 GPW_TRY(cudaGetLastError(), "brick items");
                 if ((rc = scan_counts(S, np, nbrick_all, ioff, &nbitem, st)) != GPW_OK) return rc;
