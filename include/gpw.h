@@ -45,6 +45,19 @@
  *   - eval calls are asynchronous on the given CUDA stream, allocate nothing
  *     visible to the caller and do not synchronise.  Results may differ from run to
  *     run at the 1e-15 level (floating-point atomics).
+ *   - Concurrency: the eval / interp calls write workspaces owned by the plan (pair
+ *     polynomials, pair moments, FFT scratch).  Calls on ONE plan are therefore
+ *     serialised on the device: each call makes its stream wait for the previous
+ *     call on the same plan, whichever stream that ran on, so issuing them on
+ *     different streams is safe but gives no overlap; use one plan per concurrent
+ *     pipeline.  A plan must not be used from two host threads at the same time.
+ *     The current CUDA device of an eval call must be the device the plan was built
+ *     on (GPW_EINVAL otherwise).
+ *   - Alignment: every level pointer (rho_dev[a], v_dev[a]) must be 16-byte aligned
+ *     (the kernels use 16-byte loads and stores); D_dev / F_dev 8-byte.
+ *   - Size cap: the plan holds geometry-only tables of about 112 bytes per
+ *     (pair, block) visit (gpw_info.device_bytes: 4 GB for 256 waters, 24 GB for 512
+ *     waters with f shells); gpw_build_pairs returns GPW_ENOMEM when they do not fit.
  */
 #ifndef GPW_H
 #define GPW_H
@@ -61,10 +74,13 @@ typedef struct gpw_plan gpw_plan; /* opaque; owned by the library; freed by gpw_
 typedef enum {
     GPW_OK = 0,
     GPW_EINVAL = -1,       /* null pointer, l > 3, exponent/tau <= 0, singular cell (|det| < 1e-12),
-                              mesh entry not a positive multiple of 4, deriv not in {0,1}, nlevel > 8 */
+                              mesh entry not a positive multiple of 4, a level finer than level 0 on some axis,
+                              deriv out of range, nlevel > 8, misaligned level pointer, wrong current device */
     GPW_ENOMEM = -2,
     GPW_ECUDA = -3,        /* a CUDA / cuFFT call failed, or the plan has no device copy */
-    GPW_EUNSUPPORTED = -4  /* l >= 4, more lattice wraps than the visit encoding holds */
+    GPW_EUNSUPPORTED = -4  /* l >= 4, more lattice wraps than the visit encoding holds, a pair so sharp
+                              that its Gaussian underflows inside its own grid blocks (a_p (R_t + block
+                              diagonal)^2 > 600: the mesh is far too coarse for the basis) */
 } gpw_status;
 
 /* Plan summary (host struct filled by gpw_plan_info). */
@@ -88,6 +104,13 @@ typedef struct {
     double R;                          /* pair radius R_t (T4) */
 } gpw_task;
 
+/* One (pair, lattice image, 4x4x4 block) visit of the plan's lists (host struct filled by gpw_plan_export_visits). */
+typedef struct {
+    int task;       /* index of the pair in the order of gpw_plan_export_tasks */
+    int block[3];   /* UNWRAPPED block coordinates beta_i = floor(n_i / 4) on the pair's level (T6);
+                       the stored block is beta mod (N / 4) */
+} gpw_visit;
+
 /*
  * Screening, radii, level assignment, lattice images and block lists.
  * All pointer arguments are HOST memory.
@@ -96,7 +119,8 @@ typedef struct {
  *   shl_atom    [nshl] centre index;  shl_l [nshl] 0..3;  shl_nprim [nshl] >= 1;
  *   shl_prim_off[nshl] offset of the shell's first primitive in prim_exp / prim_coef
  *   prim_exp    [nprim] Bohr^-2, > 0;  prim_coef [nprim]
- *   mesh        [nlevel][3], finest level first, every entry a positive multiple of 4
+ *   mesh        [nlevel][3], finest level first (no level may exceed level 0 on any axis), every entry a
+ *               positive multiple of 4
  *   tau         threshold of Eq. (20);  rel_cutoff  level-assignment constant (T5):
  *               a pair goes to the coarsest level with E_alpha >= rel_cutoff * a_p
  *   hermi       1: D and F symmetric, unordered pairs processed once;  0: ordered pairs
@@ -148,6 +172,10 @@ int gpw_restrict_down(gpw_plan *plan, const double *v_fine_dev, int ncomp, doubl
 int gpw_plan_info(const gpw_plan *plan, gpw_info *out);
 /* Copies up to cap tasks into host_buf (may be NULL with cap = 0); *ntask = total. */
 int gpw_plan_export_tasks(const gpw_plan *plan, gpw_task *host_buf, long cap, long *ntask);
+
+/* Copies up to cap visits of the collocation lists into host_buf (may be NULL with cap = 0); *nvisit = total.
+ * Order: level, stored block, then list order.  Reads the lists back from the device (synchronises). */
+int gpw_plan_export_visits(const gpw_plan *plan, gpw_visit *host_buf, long cap, long *nvisit);
 
 /*
  * Measurement aid: with timing enabled the eval calls bracket each of their kernels with CUDA events on

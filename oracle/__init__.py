@@ -65,6 +65,8 @@ def _load():
     L.orc_get_tasks.argtypes = [ctypes.c_void_p, _ip, _dp]
     L.orc_visit_counts.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_long)]
     L.orc_last_visit_counts.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_long)]
+    L.orc_export_visits.restype = ctypes.c_long
+    L.orc_export_visits.argtypes = [ctypes.c_void_p, ctypes.c_long, _ip]
     L.orc_eval_rho.restype = ctypes.c_int
     L.orc_eval_rho.argtypes = [ctypes.c_void_p, _dp, ctypes.c_int, ctypes.POINTER(_dp),
                                ctypes.POINTER(_ucp)]
@@ -153,6 +155,13 @@ class Oracle:
         out = np.zeros((self.nlevel, 4, 4), dtype=np.int64)
         self._L.orc_visit_counts(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_long)))
         return out
+
+    def visits(self) -> np.ndarray:
+        """ints[nvisit, 4] = task (row of tasks()), unwrapped tile coordinates beta_1, beta_2, beta_3 (T6)."""
+        n = int(self._L.orc_export_visits(self._h, 0, None))
+        buf = np.zeros((max(1, n), 4), np.int32)
+        self._L.orc_export_visits(self._h, n, _i(buf))
+        return buf[:n]
 
     def last_visit_counts(self) -> np.ndarray:
         """[nlevel,4,4] visits evaluated by the last eval_rho / eval_mat call (bookkeeping for timing)."""

@@ -397,6 +397,24 @@ static void build_visits(orc_ctx *c, const unsigned char *const *tile_mask, cons
         c->last_counts[c->task[t].level * 16 + c->task[t].la * 4 + c->task[t].lb] += c->task[t].nvis;
 }
 
+/* All (ordered task, tile) visits of T6 as rows (task index, beta_1, beta_2, beta_3) with UNWRAPPED tile
+ * coordinates; buf may be NULL (count only).  Returns the number of visits. */
+long orc_export_visits(orc_ctx *c, long cap, int *buf)
+{
+    build_visits(c, NULL, NULL);
+    long n = 0;
+    for (long t = 0; t < c->ntask; t++)
+        for (long v = 0; v < c->task[t].nvis; v++, n++)
+            if (buf && n < cap) {
+                buf[4 * n] = (int)t;
+                buf[4 * n + 1] = c->task[t].vis[3 * v];
+                buf[4 * n + 2] = c->task[t].vis[3 * v + 1];
+                buf[4 * n + 3] = c->task[t].vis[3 * v + 2];
+            }
+    clear_visits(c);
+    return n;
+}
+
 /* bookkeeping only (used to size the timed CPU baseline): visits the last eval call evaluated */
 void orc_last_visit_counts(const orc_ctx *c, long *counts)
 {

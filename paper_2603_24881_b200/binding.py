@@ -46,13 +46,20 @@ class gpw_task(ctypes.Structure):
                 ("R", ctypes.c_double)]
 
 
+class gpw_visit(ctypes.Structure):
+    _fields_ = [("task", ctypes.c_int), ("block", ctypes.c_int * 3)]
+
+
 _dp = ctypes.POINTER(ctypes.c_double)
 _ip = ctypes.POINTER(ctypes.c_int)
 _lib = None
 
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_interp_up", "gpw_restrict_down",
-           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
+           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
+
+
+__all__ = [n for n in EXPORTS if n != "gpw_last_error"] + ["GpwError", "Plan", "load_library", "model_flops", "EXPORTS"]
 
 
 def load_library():
@@ -84,6 +91,9 @@ def load_library():
     L.gpw_plan_export_tasks.restype = ctypes.c_int
     L.gpw_plan_export_tasks.argtypes = [ctypes.c_void_p, ctypes.POINTER(gpw_task), ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_long)]
+    L.gpw_plan_export_visits.restype = ctypes.c_int
+    L.gpw_plan_export_visits.argtypes = [ctypes.c_void_p, ctypes.POINTER(gpw_visit), ctypes.c_long,
+                                         ctypes.POINTER(ctypes.c_long)]
     L.gpw_plan_set_timing.restype = ctypes.c_int
     L.gpw_plan_set_timing.argtypes = [ctypes.c_void_p, ctypes.c_int]
     L.gpw_plan_get_timing.restype = ctypes.c_int
@@ -171,6 +181,16 @@ def gpw_plan_export_tasks(plan: Plan):
     return ints, R
 
 
+def gpw_plan_export_visits(plan: Plan) -> np.ndarray:
+    """ints[nvisit, 4] = task (row of gpw_plan_export_tasks), unwrapped block coordinates b1, b2, b3."""
+    L = load_library()
+    n = ctypes.c_long()
+    _check(L.gpw_plan_export_visits(plan._h, None, 0, ctypes.byref(n)))
+    buf = np.zeros((max(1, n.value), 4), np.int32)
+    _check(L.gpw_plan_export_visits(plan._h, buf.ctypes.data_as(ctypes.POINTER(gpw_visit)), n.value, ctypes.byref(n)))
+    return buf[:n.value]
+
+
 def _stream_ptr(stream) -> ctypes.c_void_p:
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
@@ -204,11 +224,17 @@ def gpw_eval_mat(plan: Plan, v: Sequence, deriv: int, F, stream=None):
 
 
 def gpw_interp_up(plan: Plan, rho: Sequence, ncomp: int, rho_fine, stream=None):
+    for lev in range(plan.nlevel):
+        _check_grid(rho[lev], (int(ncomp),) + tuple(int(x) for x in plan.mesh[lev]), f"rho[{lev}]")
+    _check_grid(rho_fine, (int(ncomp),) + tuple(int(x) for x in plan.mesh[0]), "rho_fine")
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[r.data_ptr() for r in rho])
     _check(load_library().gpw_interp_up(plan._h, ptrs, int(ncomp), ctypes.c_void_p(rho_fine.data_ptr()), _stream_ptr(stream)))
 
 
 def gpw_restrict_down(plan: Plan, v_fine, ncomp: int, v: Sequence, stream=None):
+    for lev in range(plan.nlevel):
+        _check_grid(v[lev], (int(ncomp),) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
+    _check_grid(v_fine, (int(ncomp),) + tuple(int(x) for x in plan.mesh[0]), "v_fine")
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
     _check(load_library().gpw_restrict_down(plan._h, ctypes.c_void_p(v_fine.data_ptr()), int(ncomp), ptrs, _stream_ptr(stream)))
 

@@ -302,11 +302,15 @@ template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
                    const double *rec, const double *vg, cudaStream_t st) {
     constexpr int smem = NWARP * warp_doubles(LMAX, ORTHO) * (int)sizeof(double);
-    static bool configured = false;   // per instantiation
-    if (!configured) {
+    // the attribute is per device (and per instantiation)
+    static bool configured_dev[64] = {false};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
+    const bool known = dev >= 0 && dev < 64;
+    if (!known || !configured_dev[dev]) {
         const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (known) configured_dev[dev] = true;
     }
     k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
     return cudaGetLastError();

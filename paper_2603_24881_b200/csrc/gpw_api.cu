@@ -9,9 +9,11 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "gpw_kernels.cuh"
 #include "plan_device.h"
@@ -100,6 +102,10 @@ struct gpw_plan {
     cudaEvent_t ev[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
     bool ev_valid[2] = {false, false};
     InterpState *interp = nullptr;   // cuFFT plans and scratch of gpw_interp_up / gpw_restrict_down (first use)
+    // The eval / interp calls write plan-owned workspaces (d_coef, d_mom, the interp scratch): calls on one plan are
+    // serialised on the device -- every call first makes its stream wait for `busy`, recorded at the end of the
+    // previous call on this plan, whatever stream that one ran on.
+    cudaEvent_t busy = nullptr;
 };
 
 namespace {
@@ -121,6 +127,8 @@ bool upload(T **dst, const T *src, size_t n, long &bytes, const char *what) {
 }
 
 void free_device(gpw_plan *p) {
+    if (p->busy) cudaEventDestroy(p->busy);
+    p->busy = nullptr;
     interp_free(p->interp);
     p->interp = nullptr;
     for (int w = 0; w < 2; w++)
@@ -146,6 +154,24 @@ void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
         for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[a][L];
     }
 }
+
+// Start of a call that uses the plan's device state: the current device must be the plan's, and the call's stream
+// waits for the previous call on this plan (see gpw_plan::busy).
+int begin_call(const gpw_plan *p, cudaStream_t st, const char *who) {
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), who)) return GPW_ECUDA;
+    if (dev != p->device) {
+        set_error(std::string(who) + ": the current CUDA device (" + std::to_string(dev) + ") is not the device the plan was built on (" +
+                  std::to_string(p->device) + ")");
+        return GPW_EINVAL;
+    }
+    if (!cuda_ok(cudaStreamWaitEvent(st, p->busy, 0), who)) return GPW_ECUDA;
+    return GPW_OK;
+}
+int end_call(const gpw_plan *p, cudaStream_t st, const char *who) {
+    return cuda_ok(cudaEventRecord(p->busy, st), who) ? GPW_OK : GPW_ECUDA;
+}
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace
 
@@ -249,6 +275,7 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
                  cuda_ok(cudaDeviceSynchronize(), "entry Gaussians");
         }
     }
+    ok = ok && cuda_ok(cudaEventCreateWithFlags(&p->busy, cudaEventDisableTiming), "create event");
     if (!ok) {
         free_device(p);
         delete hp;
@@ -303,14 +330,57 @@ int gpw_plan_export_tasks(const gpw_plan *p, gpw_task *buf, long cap, long *ntas
     return GPW_OK;
 }
 
+int gpw_plan_export_visits(const gpw_plan *p, gpw_visit *buf, long cap, long *nvisit) {
+    if (!p || !nvisit) { set_error("gpw_plan_export_visits: null argument"); return GPW_EINVAL; }
+    const HostPlan *hp = p->hp;
+    *nvisit = (long)hp->nvisit_total;
+    if (!buf || cap <= 0) return GPW_OK;
+    long long ntile_all = 0;
+    for (int a = 0; a < hp->nlevel; a++) ntile_all += hp->lev[a].ntile;
+    std::vector<Visit> vis;
+    std::vector<long long> base;
+    const Visit *V = nullptr;
+    if (p->on_device) {   // the lists live on the device only
+        try { vis.resize((size_t)hp->nvisit_total); base.resize((size_t)ntile_all + 1); }
+        catch (const std::bad_alloc &) { set_error("gpw_plan_export_visits: out of host memory"); return GPW_ENOMEM; }
+        if (!cuda_ok(cudaMemcpy(vis.data(), p->lists.visit, sizeof(Visit) * vis.size(), cudaMemcpyDeviceToHost), "gpw_plan_export_visits") ||
+            !cuda_ok(cudaMemcpy(base.data(), p->lists.tile_base, sizeof(long long) * base.size(), cudaMemcpyDeviceToHost), "gpw_plan_export_visits"))
+            return GPW_ECUDA;
+        V = vis.data();
+    } else {
+        for (int a = 0; a < hp->nlevel; a++) base.insert(base.end(), hp->tile_base[a].begin(), hp->tile_base[a].begin() + hp->lev[a].ntile);
+        base.push_back(hp->nvisit_total);
+        V = hp->visit.data();
+    }
+    long long tile0 = 0;
+    long n = 0;
+    for (int a = 0; a < hp->nlevel && n < cap; a++) {
+        const LevelGeom &g = hp->lev[a];
+        for (int tl = 0; tl < g.ntile && n < cap; tl++) {
+            const int w3 = tl % g.T[2], w2 = (tl / g.T[2]) % g.T[1], w1 = tl / (g.T[2] * g.T[1]);
+            for (long long i = base[tile0 + tl]; i < base[tile0 + tl + 1] && n < cap; i++, n++) {
+                buf[n].task = V[i].task;
+                buf[n].block[0] = w1 + V[i].s[0] * g.T[0];
+                buf[n].block[1] = w2 + V[i].s[1] * g.T[1];
+                buf[n].block[2] = w3 + V[i].s[2] * g.T[2];
+            }
+        }
+        tile0 += g.ntile;
+    }
+    return GPW_OK;
+}
+
 int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *const *rho_dev, void *cuda_stream) {
     if (!p || !D_dev || !rho_dev) { set_error("gpw_eval_rho: null argument"); return GPW_EINVAL; }
     if (deriv != 0 && deriv != 1) { set_error("gpw_eval_rho: deriv must be 0 or 1"); return GPW_EINVAL; }
     if (!p->on_device) { set_error("gpw_eval_rho: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     const HostPlan *hp = p->hp;
-    for (int a = 0; a < hp->nlevel; a++)
+    for (int a = 0; a < hp->nlevel; a++) {
         if (!rho_dev[a]) { set_error("gpw_eval_rho: null level pointer"); return GPW_EINVAL; }
+        if (!aligned16(rho_dev[a])) { set_error("gpw_eval_rho: level pointers must be 16-byte aligned"); return GPW_EINVAL; }
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, "gpw_eval_rho")) return rc;
     const int ncomp = deriv ? 4 : 1;
     for (int a = 0; a < hp->nlevel; a++) {
         const LevelGeom &g = hp->lev[a];
@@ -318,7 +388,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
         if (!cuda_ok(cudaMemsetAsync(rho_dev[a], 0, nb, st), "gpw_eval_rho: memset")) return GPW_ECUDA;
     }
     const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
-    if (ntask == 0 || nitem == 0) return GPW_OK;
+    if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_rho");
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[0][0], st); pm->ev_valid[0] = true; }
     k_poly_from_D<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, D_dev, hp->nao, p->d_S, p->d_coef);
@@ -329,7 +399,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
-    return GPW_OK;
+    return end_call(p, st, "gpw_eval_rho");
 }
 
 int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, double *F_dev, void *cuda_stream) {
@@ -337,12 +407,15 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     if (deriv != 0 && deriv != 1) { set_error("gpw_eval_mat: deriv must be 0 or 1"); return GPW_EINVAL; }
     if (!p->on_device) { set_error("gpw_eval_mat: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     const HostPlan *hp = p->hp;
-    for (int a = 0; a < hp->nlevel; a++)
+    for (int a = 0; a < hp->nlevel; a++) {
         if (!v_dev[a]) { set_error("gpw_eval_mat: null level pointer"); return GPW_EINVAL; }
+        if (!aligned16(v_dev[a])) { set_error("gpw_eval_mat: level pointers must be 16-byte aligned"); return GPW_EINVAL; }
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, "gpw_eval_mat")) return rc;
     if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
-    if (ntask == 0 || nitem == 0) return GPW_OK;
+    if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_mat");
     if (!cuda_ok(cudaMemsetAsync(p->d_mom, 0, sizeof(double) * (size_t)hp->ncoef_total, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     GridParams P;
     fill_params(p, P, const_cast<double *const *>(v_dev));
@@ -356,7 +429,7 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     k_F_from_moments<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, p->d_mom, p->d_S, dv, F_dev, hp->nao);
     if (p->timing) cudaEventRecord(p->ev[1][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat: kernel launch")) return GPW_ECUDA;
-    return GPW_OK;
+    return end_call(p, st, "gpw_eval_mat");
 }
 
 int gpw_plan_set_timing(gpw_plan *p, int enable) {
@@ -418,7 +491,10 @@ int gpw_interp_up(gpw_plan *p, const double *const *rho_dev, int ncomp, double *
     if (!p->on_device) { set_error("gpw_interp_up: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     for (int a = 0; a < p->hp->nlevel; a++)
         if (!rho_dev[a]) { set_error("gpw_interp_up: null level pointer"); return GPW_EINVAL; }
-    return interp_up(p->hp, &p->interp, rho_dev, ncomp, rho_fine_dev, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, "gpw_interp_up")) return rc;
+    if (const int rc = interp_up(p->hp, &p->interp, rho_dev, ncomp, rho_fine_dev, st)) return rc;
+    return end_call(p, st, "gpw_interp_up");
 }
 
 int gpw_restrict_down(gpw_plan *p, const double *v_fine_dev, int ncomp, double *const *v_dev, void *cuda_stream) {
@@ -427,7 +503,10 @@ int gpw_restrict_down(gpw_plan *p, const double *v_fine_dev, int ncomp, double *
     if (!p->on_device) { set_error("gpw_restrict_down: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     for (int a = 0; a < p->hp->nlevel; a++)
         if (!v_dev[a]) { set_error("gpw_restrict_down: null level pointer"); return GPW_EINVAL; }
-    return interp_down(p->hp, &p->interp, v_fine_dev, ncomp, v_dev, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, "gpw_restrict_down")) return rc;
+    if (const int rc = interp_down(p->hp, &p->interp, v_fine_dev, ncomp, v_dev, st)) return rc;
+    return end_call(p, st, "gpw_restrict_down");
 }
 
 }  // extern "C"

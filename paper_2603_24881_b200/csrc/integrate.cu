@@ -314,11 +314,15 @@ template <int DERIV, int LMAX, bool ORTHO>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    const double *eg, double *mom, cudaStream_t st) {
     constexpr int smem = brick_doubles(DERIV ? 4 : 1, ORTHO) * (int)sizeof(double);
-    static bool configured = false;   // per instantiation
-    if (!configured) {
+    // the attribute is per device (and per instantiation)
+    static bool configured_dev[64] = {false};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
+    const bool known = dev >= 0 && dev < 64;
+    if (!known || !configured_dev[dev]) {
         const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (known) configured_dev[dev] = true;
     }
     k_integrate<DERIV, LMAX, ORTHO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
     return cudaGetLastError();

@@ -153,6 +153,8 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
     if (hermi != 0 && hermi != 1) { set_error("gpw_build_pairs: hermi must be 0 or 1"); return GPW_EINVAL; }
     for (int i = 0; i < 3 * nlevel; i++)
         if (mesh[i] < 4 || mesh[i] % 4) { set_error("gpw_build_pairs: every mesh entry must be a positive multiple of 4"); return GPW_EINVAL; }
+    for (int i = 3; i < 3 * nlevel; i++)
+        if (mesh[i] > mesh[i % 3]) { set_error("gpw_build_pairs: level 0 must be the finest mesh on every axis (gpw_interp_up / gpw_restrict_down embed every level's spectrum in level 0's)"); return GPW_EINVAL; }
     int nprim = 0;
     for (int s = 0; s < nshl; s++) {
         if (shl_l[s] < 0) { set_error("gpw_build_pairs: negative angular momentum"); return GPW_EINVAL; }
@@ -221,6 +223,17 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             for (int k = 3; k < 6; k++)
                 if (hp->lev[a].Gm[k] != 0.0) hp->ortho = false;
 
+        // circumradius of a block about its centre (points at +-1.5 steps per axis)
+        for (int a = 0; a < nlevel; a++) {
+            double m = 0;
+            for (int sg = 0; sg < 4; sg++) {
+                double v[3];
+                for (int x = 0; x < 3; x++)
+                    v[x] = 1.5 * (hp->lev[a].H[x * 3 + 0] + ((sg & 1) ? -1 : 1) * hp->lev[a].H[x * 3 + 1] + ((sg & 2) ? -1 : 1) * hp->lev[a].H[x * 3 + 2]);
+                m = std::max(m, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+            }
+            hp->circ[a] = m;
+        }
         // ---- T1 radii ----
         std::vector<double> prad(nprim, 0.0);
         std::vector<int> prim_shl(nprim, -1);
@@ -236,6 +249,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         if (nthread < 1) nthread = 1;
         if (nthread > 64) nthread = 64;
         std::vector<std::vector<HostTask>> per_shell(nshl);
+        std::atomic<int> too_sharp(0);
         parallel_chunks(nshl, 1, nthread, [&](long, long lo, long hi, int) {
             for (long sa = lo; sa < hi; sa++) {
                 std::vector<HostTask> &outv = per_shell[sa];
@@ -286,6 +300,12 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                                         int lev = 0;
                                         for (int a = nlevel - 1; a >= 0; a--)
                                             if (hp->lev[a].ecut >= rel_cutoff * ap) { lev = a; break; }
+                                        // The kernels anchor the Gaussian recursion (Eq. 24-25) at the corner of a visited block: its
+                                        // value there, exp(-a_p d^2) with d up to R + one block diagonal, must not underflow.
+                                        {
+                                            const double reach = R + 2.0 * hp->circ[lev];
+                                            if (ap * reach * reach > 600.0) { too_sharp = 1; continue; }
+                                        }
                                         t.shl_a = (int)sa; t.prim_a = pa; t.shl_b = sb; t.prim_b = pb;
                                         t.T[0] = t0; t.T[1] = t1; t.T[2] = t2;
                                         t.level = lev; t.la = shl_l[sa]; t.lb = shl_l[sb];
@@ -297,6 +317,12 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                         }
             }
         });
+        if (too_sharp) {
+            delete hp;
+            set_error("gpw_build_pairs: a primitive pair is far too sharp for the finest mesh (a_p (R_t + block diagonal)^2 > 600: "
+                      "the Gaussian underflows at the corner of its own grid blocks); use a finer level 0");
+            return GPW_EUNSUPPORTED;
+        }
         size_t nt = 0;
         for (auto &v : per_shell) nt += v.size();
         if (nt > 2000000000ull) { delete hp; set_error("gpw_build_pairs: more than 2^31 pairs"); return GPW_EUNSUPPORTED; }
@@ -366,17 +392,6 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
         });
         hp->ncoef_total = coff;
-        // circumradius of a block about its centre (points at +-1.5 steps per axis)
-        for (int a = 0; a < nlevel; a++) {
-            double m = 0;
-            for (int sg = 0; sg < 4; sg++) {
-                double v[3];
-                for (int x = 0; x < 3; x++)
-                    v[x] = 1.5 * (hp->lev[a].H[x * 3 + 0] + ((sg & 1) ? -1 : 1) * hp->lev[a].H[x * 3 + 1] + ((sg & 2) ? -1 : 1) * hp->lev[a].H[x * 3 + 2]);
-                m = std::max(m, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
-            }
-            hp->circ[a] = m;
-        }
         if (!build_lists) {   // the block / brick lists are built on the device (plan_device.cu)
             hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
             *out = hp;

@@ -49,6 +49,24 @@ def test_argument_validation():
     expect(binding.GPW_EUNSUPPORTED, 5, np.array([4] * inp.nshl, np.int32))   # g shells
     expect(binding.GPW_EINVAL, 8, -inp.prim_exp)                          # exponent <= 0
     expect(binding.GPW_EINVAL, 14, 2)                                     # hermi
+    # a coarse level finer than level 0 on one axis (the spectrum embedding of gpw_interp_up would not fit)
+    b = list(inputs.make_small("triclinic").abi_args())
+    b[11] = np.array([[36, 32, 28], [20, 36, 16]])
+    with pytest.raises(gpw.GpwError) as e:
+        gpw.gpw_build_pairs(*b)
+    assert e.value.code == binding.GPW_EINVAL
+
+
+def test_pair_too_sharp_for_the_mesh_is_refused():
+    """A primitive so sharp that exp(-a_p d^2) underflows at the corner of its own 4x4x4 blocks would come out as
+    zeros from the corner-anchored Gaussian recursion (Eq. 24-25): gpw_build_pairs refuses it instead."""
+    cell = np.eye(3) * 8.0
+    ok = inputs.make_custom(cell, [[1.0, 2.0, 3.0]], [[(0, [40.0], [1.0])]], [[32, 32, 32]], C=np.ones((1, 1)))
+    gpw.gpw_build_pairs(*ok.abi_args())                       # a_p h^2 = 5: crude quadrature, still representable
+    sharp = inputs.make_custom(cell, [[1.0, 2.0, 3.0]], [[(0, [400.0], [1.0])]], [[32, 32, 32]], C=np.ones((1, 1)))
+    with pytest.raises(gpw.GpwError) as e:
+        gpw.gpw_build_pairs(*sharp.abi_args())
+    assert e.value.code == binding.GPW_EUNSUPPORTED and "sharp" in str(e.value)
 
 
 @pytest.mark.parametrize("kind", ["triclinic", "ortho", "wrap", "contracted"])
@@ -83,6 +101,29 @@ def test_plan_matches_oracle_enumeration(kind):
     osym = ocnt + np.transpose(ocnt, (0, 2, 1))
     self_visits = 2 * sym - osym
     assert (self_visits >= 0).all() and int(self_visits.sum()) > 0 and int(self_visits.sum()) % 2 == 0
+
+
+def visit_set(tasks_ints, visits):
+    """Sorted unique rows (shl_a, prim_a, shl_b, prim_b, T0, T1, T2, level, b1, b2, b3) of a task table and its
+    visit rows; a (pair, block) visit listed twice fails."""
+    rows = np.concatenate([np.asarray(tasks_ints)[visits[:, 0]], visits[:, 1:]], axis=1).astype(np.int64)
+    uniq = np.unique(rows, axis=0)
+    assert len(uniq) == len(rows), "a (pair, block) visit is listed twice"
+    return uniq
+
+
+@pytest.mark.parametrize("kind", ["triclinic", "wrap", "contracted"])
+def test_visit_lists_equal_oracle_visit_set(kind):
+    """Pin G12 as a SET: every (pair, lattice image, unwrapped block) triple of the plan's collocation lists is one
+    of the oracle's T6 visits and vice versa (ordered pairs).  Without a GPU this checks the host list builder;
+    tests/test_gpu_parity.py repeats it on the device-built lists."""
+    inp = inputs.make_small(kind)
+    o = oracle.Oracle.from_inputs(inp)
+    want = visit_set(o.tasks()[0], o.visits())
+    plan = _build(inp, hermi=0)
+    got = visit_set(gpw.gpw_plan_export_tasks(plan)[0], gpw.gpw_plan_export_visits(plan))
+    assert np.array_equal(got, want)
+    assert len(got) == int(o.visit_counts().sum())
 
 
 def test_eval_without_device_fails_loudly():

@@ -340,3 +340,84 @@ def test_gradient_against_fourier_derivative_and_integral_of_gradient():
     F = o.eval_mat([v], 1)
     S = overlap.periodic_overlap(inp)
     assert np.abs(F).max() < 1e-10 * np.abs(S).max()
+
+
+# ---------------------------------------------------------------- masked (sampled) evaluation
+# The full-size GPU parity tests (cfg 2-4) compare against eval_rho(tile_masks=...) / eval_mat(pair_mask=...):
+# the mask branch of task_tiles and the tile_mask / pair_mask branches of build_visits.  They are pinned here
+# against the unmasked evaluators (themselves pinned above), not against the CUDA path.
+@pytest.mark.parametrize("kind,deriv", [("triclinic", 1), ("wrap", 0), ("contracted", 1)])
+def test_masked_rho_equals_unmasked_on_marked_blocks_and_zero_elsewhere(kind, deriv):
+    inp = inputs.make_small(kind, deriv=deriv)
+    o = oracle.Oracle.from_inputs(inp)
+    D = inp.D()
+    full = o.eval_rho(D, deriv)
+    full_counts = o.last_visit_counts()
+    rng = np.random.default_rng(21)
+    masks = []
+    for lev in range(inp.nlevel):
+        T = (inp.mesh[lev] // 4).astype(int)
+        m = (rng.random(tuple(T)) < 0.3).astype(np.uint8)
+        # blocks on the cell faces are reached only through wrapped (folded) visits of pairs near the far face
+        m[0, :, -1] = 1
+        m[-1, 0, :] = 1
+        masks.append(m)
+    if inp.nlevel > 1:
+        masks[-1] = None          # a level that is not sampled at all
+    got = o.eval_rho(D, deriv, tile_masks=masks)
+    sub_counts = o.last_visit_counts()
+    assert 0 < sub_counts.sum() < full_counts.sum()
+    for lev in range(inp.nlevel):
+        if masks[lev] is None:
+            assert not np.any(got[lev])
+            assert sub_counts[lev].sum() == 0
+            continue
+        pm = np.repeat(np.repeat(np.repeat(masks[lev].astype(bool), 4, 0), 4, 1), 4, 2)
+        for c in range(full[lev].shape[0]):
+            assert np.array_equal(got[lev][c][pm], full[lev][c][pm])      # same visits, same order: bit for bit
+            assert not np.any(got[lev][c][~pm])
+        assert np.any(full[lev][0][~pm])                                    # the complement was not empty
+
+
+@pytest.mark.parametrize("kind,deriv", [("triclinic", 1), ("wrap", 0), ("contracted", 1)])
+def test_masked_mat_equals_unmasked_on_marked_shell_blocks(kind, deriv):
+    inp = inputs.make_small(kind, deriv=deriv)
+    o = oracle.Oracle.from_inputs(inp)
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    full = o.eval_mat(v, deriv)
+    full_counts = o.last_visit_counts()
+    rng = np.random.default_rng(22)
+    pmask = (rng.random((inp.nshl, inp.nshl)) < 0.35).astype(np.uint8)
+    pmask[0, inp.nshl - 1] = 1
+    pmask[inp.nshl - 1, 0] = 0            # not symmetric on purpose: (a,b) and (b,a) are separate blocks
+    got = o.eval_mat(v, deriv, pair_mask=pmask)
+    sub_counts = o.last_visit_counts()
+    assert 0 < sub_counts.sum() < full_counts.sum()
+    loc = inp.ao_loc
+    for sa in range(inp.nshl):
+        for sb in range(inp.nshl):
+            blk = (slice(loc[sa], loc[sa + 1]), slice(loc[sb], loc[sb + 1]))
+            if pmask[sa, sb]:
+                assert np.array_equal(got[blk], full[blk])
+            else:
+                assert not np.any(got[blk])
+    assert np.any(full[loc[-2]:, :loc[1]])   # the unmarked block (last shell, first shell) is not empty in the full F
+
+
+def test_masked_visit_counts_add_up_over_a_partition_of_the_blocks():
+    """The masked evaluator visits every (task, block) exactly once over a partition of the stored blocks
+    (no visit lost or doubled by the wrapped block id of the mask lookup)."""
+    inp = inputs.make_small("wrap", deriv=0)
+    o = oracle.Oracle.from_inputs(inp)
+    D = inp.D()
+    total = o.visit_counts()
+    T = (inp.mesh[0] // 4).astype(int)
+    part = np.random.default_rng(5).integers(0, 3, tuple(T))
+    acc = np.zeros_like(total)
+    rho = np.zeros((1,) + tuple(int(x) for x in inp.mesh[0]))
+    for k in range(3):
+        r = o.eval_rho(D, 0, tile_masks=[(part == k).astype(np.uint8)])
+        acc += o.last_visit_counts()
+        rho += r[0]
+    assert np.array_equal(acc, total)
+    assert np.array_equal(rho, o.eval_rho(D, 0)[0])
