@@ -72,6 +72,8 @@ def _load():
                                ctypes.POINTER(_ucp)]
     L.orc_eval_mat.restype = ctypes.c_int
     L.orc_eval_mat.argtypes = [ctypes.c_void_p, ctypes.POINTER(_dp), ctypes.c_int, _dp, _ucp]
+    L.orc_eval_grad.restype = ctypes.c_int
+    L.orc_eval_grad.argtypes = [ctypes.c_void_p, ctypes.POINTER(_dp), ctypes.c_int, _dp, _dp]
     L.orc_prim_radius.restype = ctypes.c_double
     L.orc_prim_radius.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double]
     L.orc_pair_radius.restype = ctypes.c_double
@@ -100,6 +102,9 @@ def prim_radius(l: int, a: float, coef: float, tau: float) -> float:
 
 def pair_radius(la, lb, ap, kappa, dA, dB, tau) -> float:
     return float(_load().orc_pair_radius(la, lb, ap, kappa, dA, dB, tau))
+
+
+_NCOMP = {0: 1, 1: 4, 2: 5}   # value | + gradient (T8) | + kinetic-energy density (T10)
 
 
 class Oracle:
@@ -173,7 +178,7 @@ class Oracle:
                  tile_masks: Optional[Sequence[Optional[np.ndarray]]] = None) -> List[np.ndarray]:
         D = np.ascontiguousarray(D, np.float64)
         assert D.shape == (self.nao, self.nao)
-        nc = 4 if deriv else 1
+        nc = _NCOMP[int(deriv)]
         rho = [np.zeros((nc,) + tuple(int(x) for x in m)) for m in self.mesh]
         ptrs = (_dp * self.nlevel)(*[_d(r) for r in rho])
         mptr = None
@@ -195,7 +200,7 @@ class Oracle:
 
     def eval_mat(self, v: Sequence[np.ndarray], deriv: int = 0,
                  pair_mask: Optional[np.ndarray] = None) -> np.ndarray:
-        nc = 4 if deriv else 1
+        nc = _NCOMP[int(deriv)]
         vv = []
         for lev in range(self.nlevel):
             a = np.ascontiguousarray(v[lev], np.float64)
@@ -210,3 +215,20 @@ class Oracle:
         rc = self._L.orc_eval_mat(self._h, ptrs, int(deriv), _d(F), pm)
         assert rc == 0
         return F
+
+    def eval_grad(self, v: Sequence[np.ndarray], deriv: int, D: np.ndarray) -> np.ndarray:
+        """[natm, 3] nuclear gradient of sum_alpha dV sum_r [v0 rho + w . grad rho] at fixed v, w (T11)."""
+        assert deriv in (0, 1)
+        nc = _NCOMP[int(deriv)]
+        vv = []
+        for lev in range(self.nlevel):
+            a = np.ascontiguousarray(v[lev], np.float64)
+            assert a.shape == (nc,) + tuple(int(x) for x in self.mesh[lev]), a.shape
+            vv.append(a)
+        ptrs = (_dp * self.nlevel)(*[_d(a) for a in vv])
+        D = np.ascontiguousarray(D, np.float64)
+        assert D.shape == (self.nao, self.nao)
+        g = np.zeros((self.xyz.shape[0], 3))
+        rc = self._L.orc_eval_grad(self._h, ptrs, int(deriv), _d(D), _d(g))
+        assert rc == 0
+        return g

@@ -57,7 +57,7 @@ def prim_ao_matrix(inp, level: int, deriv: int):
     binv = np.linalg.inv(cell)          # u = r @ binv ; b_i = binv[:, i]
     bnorm = np.linalg.norm(binv, axis=0)
     r = grid_points(cell, inp.mesh[level])
-    ncomp = 4 if deriv else 1
+    ncomp = 4 if deriv else 1      # deriv = 2 (tau) needs the same first derivatives as deriv = 1
     cols, exps, expand = [], [], []
     ao_loc = inp.ao_loc
     for s in range(inp.nshl):
@@ -128,6 +128,8 @@ def dense_rho(inp, D: np.ndarray, deriv: int = 0) -> List[np.ndarray]:
         if deriv:
             for c in (1, 2, 3):
                 comps.append(np.einsum("ij,ij->i", Phi[c] @ Dp, Phi[0]) + np.einsum("ij,ij->i", t, Phi[c]))
+        if deriv == 2:      # Eq. (15): tau = 1/2 sum_c diag(Phi_c D Phi_c^T)
+            comps.append(0.5 * sum(np.einsum("ij,ij->i", Phi[c] @ Dp, Phi[c]) for c in (1, 2, 3)))
         out.append(np.stack(comps).reshape(len(comps), n1, n2, n3))
     return out
 
@@ -147,6 +149,9 @@ def dense_mat(inp, v: Sequence[np.ndarray], deriv: int = 0) -> np.ndarray:
             for c in (1, 2, 3):
                 X = Phi[c].T @ (vl[c][:, None] * Phi[0])
                 Fp += X + X.T
+        if deriv == 2:      # Eq. (16) with the 1/2 of PAPER.md:265-268: 1/2 dV sum_c Phi_c^T diag(v_tau) Phi_c
+            for c in (1, 2, 3):
+                Fp += 0.5 * Phi[c].T @ (vl[4][:, None] * Phi[c])
         Fp = dV * Fp * (lev == level)
         np.add.at(F, (expand[:, None], expand[None, :]), Fp)
     return F

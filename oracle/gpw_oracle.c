@@ -19,6 +19,12 @@
  *   T7  rho(r) += sum D_ij phi_i(r) phi_j(r-T)              PAPER.md:41   Eq. (3)
  *       F_ij   += dV v(r) phi_i(r) phi_j(r-T)               PAPER.md:45   Eq. (4), dV from Eq. (29)
  *   T8  deriv=1: exact real-space gradient of Eq. (3) and Eq. (4)+(11)
+ *   T10 deriv=2 (meta-GGA): a fifth component, the kinetic-energy density
+ *       tau(r) = 1/2 sum D_ij grad phi_i . grad phi_j                     PAPER.md:100-103  Eq. (15)
+ *       F_ij  += dV v_tau(r) 1/2 grad phi_i . grad phi_j                  PAPER.md:105-107  Eq. (16) with the 1/2 of
+ *                                                                        PAPER.md:265-268 (reading A25)
+ *   T11 nuclear gradient of E = sum_alpha dV sum_r [v0 rho + w . grad rho] at fixed v, w and fixed visit set:
+ *       dE/dR_A = dV sum_r sum_ij D_ij [v0 + w . grad_r] d/dR_A (phi_i phi_j)     PAPER.md:272-309  Alg. 3
  *
  * There is no product theorem, no recursion (Eq. 24-25), no factorisation and
  * no blocking in the evaluation: phi_a and phi_b are evaluated separately with
@@ -380,6 +386,41 @@ static void shell_values(int l, double a, double coef, const double *d, int deri
         }
 }
 
+/* Second derivatives of every component of one primitive shell (needed by T11 with deriv = 1):
+ * out[i][x][y] = d^2/dx dy [x^lx y^ly z^lz e^{-a r^2}] coef, from the 1-D factors
+ *   f0 = t^l,  f1 = l t^(l-1) - 2a t^(l+1),  f2 = l(l-1) t^(l-2) - 2a(2l+1) t^l + 4a^2 t^(l+2)
+ * (each times the common Gaussian). */
+static void shell_hessian(int l, double a, double coef, const double *d, double out[][3][3])
+{
+    double e = coef * exp(-a * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+    double pw[3][ORC_MAXL + 3];
+    for (int x = 0; x < 3; x++) {
+        pw[x][0] = 1.0;
+        for (int k = 1; k <= l + 2; k++) pw[x][k] = pw[x][k - 1] * d[x];
+    }
+    int i = 0;
+    for (int lx = l; lx >= 0; lx--)
+        for (int ly = l - lx; ly >= 0; ly--) {
+            int lz = l - lx - ly;
+            int lc[3] = {lx, ly, lz};
+            double f0[3], f1[3], f2[3];
+            for (int x = 0; x < 3; x++) {
+                int n = lc[x];
+                f0[x] = pw[x][n];
+                f1[x] = -2.0 * a * pw[x][n + 1] + (n > 0 ? n * pw[x][n - 1] : 0.0);
+                f2[x] = 4.0 * a * a * pw[x][n + 2] - 2.0 * a * (2 * n + 1) * pw[x][n] + (n > 1 ? n * (n - 1) * pw[x][n - 2] : 0.0);
+            }
+            for (int x = 0; x < 3; x++)
+                for (int y = 0; y < 3; y++) {
+                    double prod = 1.0;
+                    for (int z = 0; z < 3; z++)
+                        prod *= (z == x && z == y) ? f2[z] : ((z == x || z == y) ? f1[z] : f0[z]);
+                    out[i][x][y] = prod * e;
+                }
+            i++;
+        }
+}
+
 static void build_visits(orc_ctx *c, const unsigned char *const *tile_mask, const unsigned char *pair_mask)
 {
     clear_visits(c);
@@ -427,7 +468,7 @@ void orc_last_visit_counts(const orc_ctx *c, long *counts)
  * of the array is left zero. */
 int orc_eval_rho(orc_ctx *c, const double *D, int deriv, double *const *rho, const unsigned char *const *tile_mask)
 {
-    int ncomp = deriv ? 4 : 1;
+    int ncomp = deriv == 0 ? 1 : (deriv == 1 ? 4 : 5);
     build_visits(c, tile_mask, NULL);
     for (int lev = 0; lev < c->nlevel; lev++) {
         const int *N = c->mesh + 3 * lev;
@@ -465,7 +506,7 @@ int orc_eval_rho(orc_ctx *c, const double *D, int deriv, double *const *rho, con
 #pragma omp parallel for schedule(dynamic, 4)
         for (long id = 0; id < ntile; id++) {
             if (off[id + 1] == off[id]) continue;
-            long double acc[4][64];
+            long double acc[5][64];
             memset(acc, 0, sizeof(acc));
             for (long p = off[id]; p < off[id + 1]; p++) {
                 const orc_task *k = c->task + vt[p];
@@ -487,6 +528,8 @@ int orc_eval_rho(orc_ctx *c, const double *D, int deriv, double *const *rho, con
                                     if (deriv)
                                         for (int x = 1; x < 4; x++)
                                             acc[x][pt] += (long double)(d * (fa[ia][x] * fb[ib][0] + fa[ia][0] * fb[ib][x]));
+                                    if (deriv == 2) /* Eq. (15): tau = 1/2 sum D grad phi_a . grad phi_b */
+                                        acc[4][pt] += (long double)(0.5 * d * (fa[ia][1] * fb[ib][1] + fa[ia][2] * fb[ib][2] + fa[ia][3] * fb[ib][3]));
                                 }
                         }
             }
@@ -551,6 +594,8 @@ int orc_eval_mat(orc_ctx *c, const double *const *v, int deriv, double *F, const
                                     if (deriv)
                                         for (int x = 1; x < 4; x++)
                                             s += vl[x * ng + m] * (fa[ia][x] * fb[ib][0] + fa[ia][0] * fb[ib][x]);
+                                    if (deriv == 2) /* Eq. (16) with the 1/2 of PAPER.md:265-268 */
+                                        s += vl[4 * ng + m] * 0.5 * (fa[ia][1] * fb[ib][1] + fa[ia][2] * fb[ib][2] + fa[ia][3] * fb[ib][3]);
                                     acc[ia][ib] += (long double)(dV * s);
                                 }
                         }
@@ -560,6 +605,80 @@ int orc_eval_mat(orc_ctx *c, const double *const *v, int deriv, double *F, const
                 F[(long)(k0->ao_a + ia) * c->nao + k0->ao_b + ib] = (double)acc[ia][ib];
     }
     free(gstart);
+    clear_visits(c);
+    return 0;
+}
+
+
+/* T11 nuclear gradient (Alg. 3).  E = sum_alpha dV_alpha sum_r [v0 rho_alpha + w . grad rho_alpha]
+ * with rho_alpha the collocated density of T7; v (and w for deriv = 1) are held fixed, and so is the visit set.
+ * grad[A][c] = dE/dR_{A,c}.  A basis function centred on atom A depends on R_A through r - R_A only, so
+ * d/dR_{A,c} phi_i = -d_c phi_i; for deriv = 1 the second derivatives d_x d_c phi_i enter through
+ * d/dR_{A,c} d_x (phi_i phi_j) = -(d_x d_c phi_i phi_j + d_c phi_i d_x phi_j)  (phi_i on A)
+ * and likewise for phi_j on B.  A lattice image B + T moves with B.  v[level]: [ncomp][N1][N2][N3]. */
+int orc_eval_grad(orc_ctx *c, const double *const *v, int deriv, const double *D, double *grad)
+{
+    if (deriv != 0 && deriv != 1) return -1;
+    build_visits(c, NULL, NULL);
+    int natm = c->natm;
+    int nth = orc_num_threads();
+    long double *part = (long double *)calloc((size_t)nth * 3 * natm, sizeof(long double));
+#pragma omp parallel for schedule(dynamic, 4)
+    for (long t = 0; t < c->ntask; t++) {
+#ifdef _OPENMP
+        long double *g = part + (size_t)omp_get_thread_num() * 3 * natm;
+#else
+        long double *g = part;
+#endif
+        const orc_task *k = c->task + t;
+        const int *N = c->mesh + 3 * k->level;
+        long ng = (long)N[0] * N[1] * N[2];
+        double dV = c->omega / (double)ng;
+        const double *vl = v[k->level];
+        int nca = ncart(k->la), ncb = ncart(k->lb);
+        int atom_a = c->shl_atom[k->shl_a], atom_b = c->shl_atom[k->shl_b];
+        double fa[ORC_MAXNC][4], fb[ORC_MAXNC][4], ha[ORC_MAXNC][3][3], hb[ORC_MAXNC][3][3];
+        for (long p = 0; p < k->nvis; p++)
+            for (int i = 0; i < 4; i++)
+                for (int j = 0; j < 4; j++)
+                    for (int q = 0; q < 4; q++) {
+                        int n1 = 4 * k->vis[3 * p] + i, n2 = 4 * k->vis[3 * p + 1] + j, n3 = 4 * k->vis[3 * p + 2] + q;
+                        double r[3], da[3], db[3];
+                        grid_pos(c, N, n1, n2, n3, r);
+                        for (int x = 0; x < 3; x++) { da[x] = r[x] - k->A[x]; db[x] = r[x] - k->Bt[x]; }
+                        shell_values(k->la, k->aa, k->ca, da, 1, fa);
+                        shell_values(k->lb, k->ab, k->cb, db, 1, fb);
+                        if (deriv) {
+                            shell_hessian(k->la, k->aa, k->ca, da, ha);
+                            shell_hessian(k->lb, k->ab, k->cb, db, hb);
+                        }
+                        long m = ((long)posmod(n1, N[0]) * N[1] + posmod(n2, N[1])) * N[2] + posmod(n3, N[2]);
+                        double v0 = vl[m];
+                        for (int ia = 0; ia < nca; ia++)
+                            for (int ib = 0; ib < ncb; ib++) {
+                                double d = D[(long)(k->ao_a + ia) * c->nao + k->ao_b + ib] * dV;
+                                for (int cc = 0; cc < 3; cc++) {
+                                    /* d/dR_A: phi_a -> -d_c phi_a ;  d/dR_B: phi_b -> -d_c phi_b */
+                                    double ga = -v0 * fa[ia][1 + cc] * fb[ib][0];
+                                    double gb = -v0 * fa[ia][0] * fb[ib][1 + cc];
+                                    if (deriv)
+                                        for (int x = 0; x < 3; x++) {
+                                            double w = vl[(1 + x) * ng + m];
+                                            ga -= w * (ha[ia][x][cc] * fb[ib][0] + fa[ia][1 + cc] * fb[ib][1 + x]);
+                                            gb -= w * (fa[ia][1 + x] * fb[ib][1 + cc] + fa[ia][0] * hb[ib][x][cc]);
+                                        }
+                                    g[3 * atom_a + cc] += (long double)(d * ga);
+                                    g[3 * atom_b + cc] += (long double)(d * gb);
+                                }
+                            }
+                    }
+    }
+    for (int i = 0; i < 3 * natm; i++) {
+        long double s = 0;
+        for (int th = 0; th < nth; th++) s += part[(size_t)th * 3 * natm + i];
+        grad[i] = (double)s;
+    }
+    free(part);
     clear_visits(c);
     return 0;
 }

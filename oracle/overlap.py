@@ -41,8 +41,11 @@ def overlap_1d(la: int, lb: int, a: float, b: float, A: float, B: float) -> np.n
     return S[: la + 1, : lb + 1]
 
 
-def periodic_overlap(inp, eps: float = 1e-24) -> np.ndarray:
-    """S^per[nao, nao] for the contracted Cartesian basis of ``inp``."""
+def periodic_overlap(inp, eps: float = 1e-24, kinetic: bool = False) -> np.ndarray:
+    """S^per[nao, nao] for the contracted Cartesian basis of ``inp``; with kinetic=True the periodic
+    kinetic-energy matrix T^per = sum_T 1/2 <grad phi_mu | grad phi_nu^T> instead (textbook: per axis
+    D_ij = int (d/dx g_i)(d/dx g_j) = i j S_{i-1,j-1} - 2b i S_{i-1,j+1} - 2a j S_{i+1,j-1} + 4ab S_{i+1,j+1},
+    T = 1/2 (D_x S_y S_z + S_x D_y S_z + S_x S_y D_z)) -- the pin of Eq. (15)-(16) with v_tau = 1."""
     cell = np.asarray(inp.cell, float)
     binv = np.linalg.inv(cell)
     bnorm = np.linalg.norm(binv, axis=0)
@@ -74,11 +77,23 @@ def periodic_overlap(inp, eps: float = 1e-24) -> np.ndarray:
                         for t2 in range(lo[1], hi[1] + 1):
                             for t3 in range(lo[2], hi[2] + 1):
                                 Bt = B + t1 * cell[0] + t2 * cell[1] + t3 * cell[2]
-                                sx = overlap_1d(la, lb, a, b, A[0], Bt[0])
-                                sy = overlap_1d(la, lb, a, b, A[1], Bt[1])
-                                sz = overlap_1d(la, lb, a, b, A[2], Bt[2])
-                                blk += ca * cb * (sx[np.ix_(pax[:, 0], pbx[:, 0])] *
-                                                  sy[np.ix_(pax[:, 1], pbx[:, 1])] *
-                                                  sz[np.ix_(pax[:, 2], pbx[:, 2])])
+                                s1 = [overlap_1d(la + 1, lb + 1, a, b, A[x], Bt[x]) for x in range(3)]
+                                sx, sy, sz = (t[: la + 1, : lb + 1] for t in s1)
+                                if not kinetic:
+                                    blk += ca * cb * (sx[np.ix_(pax[:, 0], pbx[:, 0])] *
+                                                      sy[np.ix_(pax[:, 1], pbx[:, 1])] *
+                                                      sz[np.ix_(pax[:, 2], pbx[:, 2])])
+                                    continue
+                                d1 = []
+                                for x in range(3):
+                                    S1 = np.pad(s1[x], ((1, 0), (1, 0)))       # S1[i + 1, j + 1] = S_ij, S_{-1,.} = 0
+                                    i = np.arange(la + 1)[:, None]
+                                    j = np.arange(lb + 1)[None, :]
+                                    d1.append(i * j * S1[i, j] - 2 * b * i * S1[i, j + 2] - 2 * a * j * S1[i + 2, j]
+                                              + 4 * a * b * S1[i + 2, j + 2])
+                                pick = lambda t, x: t[np.ix_(pax[:, x], pbx[:, x])]
+                                blk += 0.5 * ca * cb * (pick(d1[0], 0) * pick(sy, 1) * pick(sz, 2) +
+                                                        pick(sx, 0) * pick(d1[1], 1) * pick(sz, 2) +
+                                                        pick(sx, 0) * pick(sy, 1) * pick(d1[2], 2))
             S[ao_loc[sa]:ao_loc[sa + 1], ao_loc[sb]:ao_loc[sb + 1]] = blk
     return S

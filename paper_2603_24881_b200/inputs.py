@@ -95,7 +95,8 @@ class GPWInputs:
 
     @property
     def ncomp(self) -> int:
-        return 4 if self.deriv else 1
+        """Grid components: value | value + gradient | value + gradient + kinetic-energy density."""
+        return {0: 1, 1: 4, 2: 5}[int(self.deriv)]
 
     def D(self) -> np.ndarray:
         return np.ascontiguousarray(self.C @ self.C.T)
@@ -113,7 +114,11 @@ class GPWInputs:
             out[0] = self.v_const
             return out
         rng = np.random.default_rng([self.seed, 7000 + level])
-        return rng.standard_normal((4, n1, n2, n3))[:nc].copy()
+        out = rng.standard_normal((4, n1, n2, n3))[:nc].copy()
+        if nc == 5:   # the meta-GGA component has its own stream, so that components 0..3 do not depend on deriv
+            rng5 = np.random.default_rng([self.seed, 9000 + level])
+            out = np.concatenate([out, rng5.standard_normal((1, n1, n2, n3))])
+        return out
 
     def abi_args(self):
         """Positional arguments of gpw_build_pairs up to (and excluding) plan_out."""
