@@ -18,6 +18,12 @@
  *                     weight of Eq. (29) PAPER.md:185 / Alg. 2 PAPER.md:240-263;
  *                     deriv=1 adds the Eq. (11) term sum_r w(r) . grad(phi_mu phi_nu)
  *                     (before the integration by parts of Eq. 13).
+ *                     deriv=2 (meta-GGA) adds a fifth component to both: the kinetic-energy
+ *                     density tau = 1/2 sum D grad phi_mu . grad phi_nu (Eq. 15)
+ *                     and the term dV sum_r v_tau(r) 1/2 grad phi_mu . grad phi_nu of the Fock
+ *                     matrix (Eq. 16, with the 1/2 of PAPER.md:265-268).
+ *   gpw_eval_grad     nuclear gradient of the grid energy at fixed potential (Alg. 3,
+ *                     PAPER.md:272-309).
  *   gpw_interp_up / gpw_restrict_down
  *                     inter-level Fourier combination, Eq. (7)-(8) PAPER.md:61-68
  *                     (cuFFT, off the optimisation target).
@@ -36,8 +42,8 @@
  *     (s; x y z; xx xy xz yy yz zz; xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz; A2).
  *   - Grids (PAPER.md:483 with u0 = 0): level alpha has mesh (N1,N2,N3), points
  *     r_n = (n1/N1) a1 + (n2/N2) a2 + (n3/N3) a3; arrays are [ncomp][N1][N2][N3]
- *     doubles, C order (n3 fastest), ncomp = 1 (deriv=0) or 4 (deriv=1: value,
- *     d/dx, d/dy, d/dz; component-major).
+ *     doubles, C order (n3 fastest), ncomp = 1 (deriv=0), 4 (deriv=1: value,
+ *     d/dx, d/dy, d/dz; component-major) or 5 (deriv=2: those four, then tau / v_tau).
  *   - Truncation (T1-T7): a primitive pair is evaluated on all 64 points
  *     of every aligned 4x4x4 grid block that has at least one point within the pair
  *     radius R_t of the Gaussian-product centre; out-of-cell blocks are folded back
@@ -135,7 +141,8 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
                     double tau, double rel_cutoff, int hermi, gpw_plan **plan_out);
 
 /*
- * Collocation.  D_dev: DEVICE [nao][nao] row-major (read only).  deriv: 0 or 1.
+ * Collocation.  D_dev: DEVICE [nao][nao] row-major (read only).  deriv: 0, 1 or 2 (the first call with
+ * deriv = 2 allocates the plan's degree-(L+2) workspace).
  * rho_dev: HOST array of nlevel DEVICE pointers, each [ncomp][N1][N2][N3]; every level
  * is OVERWRITTEN (levels without pairs are zero-filled).  cuda_stream: a cudaStream_t
  * (NULL = default stream).  With hermi = 1 the pair (a,b) uses D_ab + D_ba, so the
@@ -149,10 +156,21 @@ int gpw_eval_rho(const gpw_plan *plan, const double *D_dev, int deriv, double *c
  * (component 0 = v, components 1..3 = the vector field w contracted with
  * grad(phi_mu phi_nu)).  F_dev: DEVICE [nao][nao] row-major, OVERWRITTEN, includes
  * dV = Omega / (N1 N2 N3) of each level and the sum over levels.  With hermi = 1 both
- * triangles are written.
+ * triangles are written.  deriv = 2: component 4 = v_tau, contracted with 1/2 grad phi_mu . grad phi_nu.
  */
 int gpw_eval_mat(const gpw_plan *plan, const double *const *v_dev, int deriv, double *F_dev,
                  void *cuda_stream);
+
+/*
+ * Nuclear gradient (Alg. 3) of the grid energy
+ *     E = sum_alpha dV_alpha sum_r [ v0(r) rho_alpha(r) + w(r) . grad rho_alpha(r) ]
+ * at FIXED v0, w and fixed visit set, rho_alpha being the collocated density of gpw_eval_rho:
+ *     grad[A][c] = dE / dR_{A,c},   d/dR_A phi(r - R_A) = -grad_r phi   (a lattice image moves with its atom).
+ * v_dev as in gpw_eval_mat with deriv = 0 (v0 only) or 1 (v0 and w); D_dev: DEVICE [nao][nao];
+ * grad_dev: DEVICE [natm][3], OVERWRITTEN.  The first call allocates the plan's degree-(L+1) workspace.
+ */
+int gpw_eval_grad(gpw_plan *plan, const double *const *v_dev, int deriv, const double *D_dev, double *grad_dev,
+                  void *cuda_stream);
 
 /*
  * Off-target helpers (cuFFT), Eq. (7)-(8):

@@ -8,6 +8,7 @@ or no CUDA device is present the eval calls raise.
                            prim_exp, prim_coef, nlevel, mesh, tau, rel_cutoff, hermi)
     gpw_eval_rho(plan, D, deriv, rho_levels)      # torch CUDA float64 tensors, rho overwritten
     gpw_eval_mat(plan, v_levels, deriv, F)        # F overwritten
+    gpw_eval_grad(plan, v_levels, deriv, D, grad) # grad [natm, 3] overwritten
 """
 from __future__ import annotations
 
@@ -50,11 +51,12 @@ class gpw_visit(ctypes.Structure):
     _fields_ = [("task", ctypes.c_int), ("block", ctypes.c_int * 3)]
 
 
+NCOMP = {0: 1, 1: 4, 2: 5}   # components of a level array per deriv (include/gpw.h)
 _dp = ctypes.POINTER(ctypes.c_double)
 _ip = ctypes.POINTER(ctypes.c_int)
 _lib = None
 
-EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_interp_up", "gpw_restrict_down",
+EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_eval_grad", "gpw_interp_up", "gpw_restrict_down",
            "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
@@ -80,6 +82,9 @@ def load_library():
     L.gpw_eval_mat.restype = ctypes.c_int
     L.gpw_eval_mat.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
                                ctypes.c_void_p, ctypes.c_void_p]
+    L.gpw_eval_grad.restype = ctypes.c_int
+    L.gpw_eval_grad.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
+                                ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
     L.gpw_interp_up.restype = ctypes.c_int
     L.gpw_interp_up.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
                                 ctypes.c_void_p, ctypes.c_void_p]
@@ -205,7 +210,7 @@ def _check_grid(t, shape, what):
 
 def gpw_eval_rho(plan: Plan, D, deriv: int, rho: Sequence, stream=None):
     """rho[level] (CUDA float64 [ncomp, N1, N2, N3]) is overwritten with the collocated density."""
-    nc = 4 if deriv else 1
+    nc = NCOMP[int(deriv)]
     _check_grid(D, (plan.nao, plan.nao), "D")
     for lev in range(plan.nlevel):
         _check_grid(rho[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"rho[{lev}]")
@@ -215,12 +220,25 @@ def gpw_eval_rho(plan: Plan, D, deriv: int, rho: Sequence, stream=None):
 
 def gpw_eval_mat(plan: Plan, v: Sequence, deriv: int, F, stream=None):
     """F (CUDA float64 [nao, nao]) is overwritten with the integrated matrix (includes dV)."""
-    nc = 4 if deriv else 1
+    nc = NCOMP[int(deriv)]
     _check_grid(F, (plan.nao, plan.nao), "F")
     for lev in range(plan.nlevel):
         _check_grid(v[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
     _check(load_library().gpw_eval_mat(plan._h, ptrs, int(deriv), ctypes.c_void_p(F.data_ptr()), _stream_ptr(stream)))
+
+
+def gpw_eval_grad(plan: Plan, v: Sequence, deriv: int, D, grad, stream=None):
+    """grad (CUDA float64 [natm, 3]) is overwritten with dE/dR of E = sum dV [v0 rho + w . grad rho] at fixed v, w."""
+    nc = NCOMP[int(deriv)]
+    _check_grid(D, (plan.nao, plan.nao), "D")
+    if not (grad.is_cuda and grad.is_contiguous() and grad.dim() == 2 and grad.shape[1] == 3 and str(grad.dtype) == "torch.float64"):
+        raise ValueError("grad: need a contiguous CUDA float64 tensor of shape [natm, 3]")
+    for lev in range(plan.nlevel):
+        _check_grid(v[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
+    ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
+    _check(load_library().gpw_eval_grad(plan._h, ptrs, int(deriv), ctypes.c_void_p(D.data_ptr()),
+                                        ctypes.c_void_p(grad.data_ptr()), _stream_ptr(stream)))
 
 
 def gpw_interp_up(plan: Plan, rho: Sequence, ncomp: int, rho_fine, stream=None):

@@ -68,9 +68,11 @@ __device__ __forceinline__ int visit_wrap(unsigned long long r, int axis) {
 
 // The group's four lanes copy the record of `task` (class L) into a slot, 16 bytes per lane and trip.
 // ... and the visit's Gaussian values (visit index iv relative to the item's first visit).
+// LMAX here is the largest polynomial degree of the instantiation, deg the degree of this pair's polynomial (the
+// pair's L plus the degree offset of the launch), L the pair's own la + lb (its class in coef_base).
 template <int LMAX, bool ORTHO>
-__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int task, unsigned iv, double *slot) {
-    const int nrec = 8 + ncoef_pad(L);          // doubles, even
+__device__ __forceinline__ void stage_visit(const ColCtx &c, int L, int deg, int task, unsigned iv, double *slot) {
+    const int nrec = 8 + ncoef_pad(deg);        // doubles, even
     const char *src = reinterpret_cast<const char *>(c.rec + c.coef_base[L] + (long long)task * nrec) + 16 * c.x;
     const unsigned dst = smem_u32(slot) + 16 * c.x;
     const int n16 = nrec / 2 - c.x;             // 16-byte units left for this lane, stride 4
@@ -124,15 +126,19 @@ __device__ __forceinline__ int group_reduce_scatter(double *a, int lane) {
     return off;
 }
 
-template <int DERIV, int LMAX, bool ORTHO>
+// LMAX: largest la + lb of the plan's pairs held by the instantiation.  LOFF: degree offset -- the polynomial of a pair
+// of class L has degree L + LOFF (0: density and gradient; 2: kinetic-energy density, Eq. 15, whose pair product is
+// again a polynomial times the same Gaussian, of degree L + 2).
+template <int DERIV, int LMAX, bool ORTHO, int LOFF>
 __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_collocate(const __grid_constant__ GridParams P,
                                                                    const Visit *__restrict__ visits,
                                                                    const Item *__restrict__ items, int nitem,
                                                                    const double *__restrict__ rec,
                                                                    const double *__restrict__ vg) {
     constexpr int NCOMP = DERIV ? 4 : 1;
-    constexpr int SLOT = slot_doubles(LMAX, ORTHO);
-    constexpr int GSTRIDE = group_stride(LMAX, ORTHO);
+    constexpr int DMAX = LMAX + LOFF;
+    constexpr int SLOT = slot_doubles(DMAX, ORTHO);
+    constexpr int GSTRIDE = group_stride(DMAX, ORTHO);
     extern __shared__ __align__(16) double sm[];
     const int warp = threadIdx.x >> 5;
     const int w = blockIdx.x * NWARP + warp;
@@ -140,7 +146,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     const Item it = items[w];
     const LevelGeom &g = P.lev[it.level];
     const int lane = threadIdx.x & 31, grp = lane >> 2, x = lane & 3;
-    double *wsm = sm + (size_t)warp * warp_doubles(LMAX, ORTHO);
+    double *wsm = sm + (size_t)warp * warp_doubles(DMAX, ORTHO);
     uint2 *tab = reinterpret_cast<uint2 *>(wsm + NGRP * GSTRIDE);
     unsigned long long *vis = reinterpret_cast<unsigned long long *>(wsm + NGRP * GSTRIDE + MAXCH);
 
@@ -201,7 +207,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     auto stage_chunk = [&](int k, int slot) {
         const uint2 e = tab[min(k, nch - 1)];
         const unsigned iv = e.x + ((unsigned)grp < (e.y >> 8) ? grp : 0);
-        stage_visit<LMAX, ORTHO>(c, (int)(e.y & 0xffu), visit_task(vis[iv]), iv, c.slot + slot * SLOT);
+        stage_visit<DMAX, ORTHO>(c, (int)(e.y & 0xffu), (int)(e.y & 0xffu) + LOFF, visit_task(vis[iv]), iv, c.slot + slot * SLOT);
         cp_async_commit();
     };
     stage_chunk(0, 0);
@@ -227,7 +233,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
             const bool valid_n = (unsigned)grp < (en.y >> 8);
             const int gi_n = valid_n ? grp : 0;
             const unsigned long long v_n = vis[en.x + gi_n];
-            colloc_visit<L, LMAX, DERIV, ORTHO>(c, v0, wsm + (size_t)gi * GSTRIDE + slot * SLOT, valid, acc);
+            colloc_visit<L + LOFF, DMAX, DERIV, ORTHO>(c, v0, wsm + (size_t)gi * GSTRIDE + slot * SLOT, valid, acc);
             valid = valid_n; gi = gi_n; v0 = v_n;
             if (++slot == NSLOT) slot = 0;
         }
@@ -253,13 +259,13 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
                 const unsigned long long v0 = vis[e.x + grp];
                 const double *s = c.slot + slot * SLOT;
                 switch ((int)(e.y & 0xffu)) {
-                    case 0: colloc_visit<0, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 1: colloc_visit<1, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 2: colloc_visit<2, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 3: colloc_visit<3, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 4: colloc_visit<4, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 5: colloc_visit<5, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    default: colloc_visit<6, LMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 0: colloc_visit<0 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 1: colloc_visit<1 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 2: colloc_visit<2 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 3: colloc_visit<3 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 4: colloc_visit<4 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 5: colloc_visit<5 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    default: colloc_visit<6 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
                 }
             }
             if (++slot == NSLOT) slot = 0;
@@ -298,36 +304,47 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     }
 }
 
-template <int DERIV, int LMAX, bool ORTHO>
+template <int DERIV, int LMAX, bool ORTHO, int LOFF>
 cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
                    const double *rec, const double *vg, cudaStream_t st) {
-    constexpr int smem = NWARP * warp_doubles(LMAX, ORTHO) * (int)sizeof(double);
+    constexpr int smem = NWARP * warp_doubles(LMAX + LOFF, ORTHO) * (int)sizeof(double);
     // the attribute is per device (and per instantiation)
     static bool configured_dev[64] = {false};
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
     const bool known = dev >= 0 && dev < 64;
     if (!known || !configured_dev[dev]) {
-        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO, LOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (known) configured_dev[dev] = true;
     }
-    k_collocate<DERIV, LMAX, ORTHO><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
+    k_collocate<DERIV, LMAX, ORTHO, LOFF><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
     return cudaGetLastError();
 }
 
 template <int DERIV, bool ORTHO>
 cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items, int nitem,
                      const double *rec, const double *vg, int max_L, cudaStream_t st) {
-    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, visits, items, nitem, rec, vg, st);
-    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, visits, items, nitem, rec, vg, st);
-    return launch<DERIV, 6, ORTHO>(P, visits, items, nitem, rec, vg, st);
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+    return launch<DERIV, 6, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+}
+// kinetic-energy density: value only, polynomials of degree L + 2
+template <bool ORTHO>
+cudaError_t launch_tau(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                       const double *rec, const double *vg, int max_L, cudaStream_t st) {
+    if (max_L <= 4) return launch<0, 4, ORTHO, 2>(P, visits, items, nitem, rec, vg, st);
+    return launch<0, 6, ORTHO, 2>(P, visits, items, nitem, rec, vg, st);
 }
 
 }  // namespace
 
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                             const double *rec, const double *vg, int deriv, int max_L, bool ortho, cudaStream_t st) {
+                             const double *rec, const double *vg, int deriv, int off, int max_L, bool ortho, cudaStream_t st) {
+    if (off == 2 && deriv == 0)
+        return ortho ? launch_tau<true>(P, visits, items, nitem, rec, vg, max_L, st)
+                     : launch_tau<false>(P, visits, items, nitem, rec, vg, max_L, st);
+    if (off != 0) return cudaErrorInvalidValue;
     if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, rec, vg, max_L, st)
                             : launch_l<1, false>(P, visits, items, nitem, rec, vg, max_L, st);
     return ortho ? launch_l<0, true>(P, visits, items, nitem, rec, vg, max_L, st)

@@ -1,10 +1,10 @@
 // The C ABI of include/gpw.h, the pre/post-pass kernels and the FP64 peak probe (sm_100a).
 //
 // Kernels:
-//   k_poly_from_D       pre-pass: one thread per pair, D block -> polynomial about P in grid-index coordinates
+//   k_pair_pass         pairpass.cu: pre-pass (D block -> pair polynomial about P in grid-index coordinates) and
+//                       post-pass (pair moments -> F block x dV, or atom gradients), eight lanes per pair
 //   k_collocate         collocate.cu
 //   k_integrate         integrate.cu
-//   k_F_from_moments    post-pass: one thread per pair, moments -> F block (x dV), atomics into F
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -16,49 +16,22 @@
 #include <vector>
 
 #include "gpw_kernels.cuh"
+#include "pairpass.cuh"
 #include "plan_device.h"
 
 namespace gpw {
 const char *last_error_cstr();
 
-// ------------------------------------------------------------------------------------------ pre/post pass
-__global__ void __launch_bounds__(128) k_poly_from_D(const TaskP *__restrict__ tp, int ntask,
-                                                      const double *__restrict__ D, int nao,
-                                                      const double *__restrict__ S_all, double *__restrict__ coef) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntask) return;
-    const TaskP p = tp[t];
-    // the pair's record in the collocation workspace: 8-double header, then the polynomial
-    pair_poly_from_D(p, D, nao, S_all + (size_t)p.level * S_TOTAL, coef + p.coef_off + 8 * (long long)t + 8);
-}
-
-// header of every pair's record in the collocation workspace (plan time)
-__global__ void __launch_bounds__(128) k_rec_headers(const TaskK *__restrict__ tk, int ntask, double *__restrict__ rec) {
+// header of every pair's record in a collocation workspace (plan time / first use): the polynomial of degree
+// L + off follows it, rewritten by every call
+__global__ void __launch_bounds__(128) k_rec_headers(const TaskK *__restrict__ tk, const TaskP *__restrict__ tp, int ntask,
+                                                     pp::PassArgs A, int off, double *__restrict__ rec) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntask) return;
     const TaskK k = tk[t];
-    double *h = rec + k.coef_off + 8 * (long long)t;
+    const int L = tp[t].la + tp[t].lb, level = tp[t].level;
+    double *h = rec + A.base[off][level][L] + (long long)t * (ncoef_pad(L + off) + 8);
     h[0] = k.nP[0]; h[1] = k.nP[1]; h[2] = k.nP[2]; h[3] = k.ap; h[4] = k.c22; h[5] = k.c23; h[6] = k.c33; h[7] = 0.0;
-}
-
-struct DVs { double v[GPW_MAX_LEVEL]; };
-
-__global__ void __launch_bounds__(128) k_F_from_moments(const TaskP *__restrict__ tp, int ntask,
-                                                         const double *__restrict__ mom,
-                                                         const double *__restrict__ S_all, DVs dV,
-                                                         double *__restrict__ F, int nao) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntask) return;
-    const TaskP p = tp[t];
-    double blk[ncart(MAXL) * ncart(MAXL)];
-    pair_block_from_moments(p, mom + p.coef_off, S_all + (size_t)p.level * S_TOTAL, dV.v[p.level], blk);
-    const int nca = ncart(p.la), ncb = ncart(p.lb);
-    for (int i = 0; i < nca; i++)
-        for (int j = 0; j < ncb; j++) {
-            const double x = blk[i * ncb + j];
-            atomicAdd(F + (size_t)(p.ao_a + i) * nao + p.ao_b + j, x);
-            if (p.sym) atomicAdd(F + (size_t)(p.ao_b + j) * nao + p.ao_a + i, x);
-        }
 }
 
 // ------------------------------------------------------------------------------------------ FP64 peak probe
@@ -93,8 +66,9 @@ struct gpw_plan {
     TaskP *d_taskP = nullptr;
     DeviceLists lists;          // visit / brick lists and work items, built on the device (plan_device.cu)
     double *d_S = nullptr;
-    double *d_coef = nullptr;   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
-    double *d_mom = nullptr;    // moment workspace of gpw_eval_mat
+    // per degree offset (0: Eq. 3-4; 1: nuclear gradient; 2: kinetic-energy density); offsets 1, 2 allocated on first use
+    double *d_coef[NOFF] = {nullptr, nullptr, nullptr};   // per-pair records of gpw_eval_rho: header (static) + polynomial (written per call)
+    double *d_mom[NOFF] = {nullptr, nullptr, nullptr};    // moment workspaces of gpw_eval_mat / gpw_eval_grad
     double *d_vg = nullptr;     // Gaussian values of every (pair, block) visit (geometry only; written at build time)
     double *d_eg = nullptr;     // 1-D Gaussian factor tables of every brick entry (orthogonal cells; geometry only)
     // optional kernel timing (gpw_plan_set_timing): events around each kernel of the last eval calls
@@ -135,11 +109,12 @@ void free_device(gpw_plan *p) {
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
     cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_S);
-    cudaFree(p->d_coef); cudaFree(p->d_mom); cudaFree(p->d_vg); cudaFree(p->d_eg);
+    for (int off = 0; off < NOFF; off++) { cudaFree(p->d_coef[off]); cudaFree(p->d_mom[off]); }
+    cudaFree(p->d_vg); cudaFree(p->d_eg);
     free_device_lists(&p->lists);
 }
 
-void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
+void fill_params(const gpw_plan *p, GridParams &P, double *const *grids, int off = 0, size_t comp = 0) {
     std::memset(&P, 0, sizeof(P));
     const HostPlan *hp = p->hp;
     long long tile0 = 0, brick0 = 0;
@@ -150,8 +125,9 @@ void fill_params(const gpw_plan *p, GridParams &P, double *const *grids) {
         P.seg[a] = p->lists.seg + tile0 * 8;
         P.brick_base[a] = p->lists.brick_base + brick0;
         tile0 += hp->lev[a].ntile; brick0 += hp->lev[a].nbrick;
-        P.grid[a] = grids[a];
-        for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[a][L];
+        // comp: the launch works on component `comp` of every level's array (the fifth component of deriv = 2)
+        P.grid[a] = grids[a] ? grids[a] + comp * (size_t)hp->lev[a].N[0] * hp->lev[a].N[1] * hp->lev[a].N[2] : nullptr;
+        for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[off][a][L];
     }
 }
 
@@ -172,6 +148,44 @@ int end_call(const gpw_plan *p, cudaStream_t st, const char *who) {
     return cuda_ok(cudaEventRecord(p->busy, st), who) ? GPW_OK : GPW_ECUDA;
 }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+void fill_pass(const gpw_plan *p, pp::PassArgs &A, int mode) {
+    std::memset(&A, 0, sizeof(A));
+    const HostPlan *hp = p->hp;
+    A.tp = p->d_taskP; A.ntask = (int)hp->task.size(); A.nao = hp->nao; A.hdiag = hp->hdiag ? 1 : 0; A.mode = mode;
+    A.S_all = p->d_S;
+    for (int off = 0; off < NOFF; off++) {
+        for (int a = 0; a < GPW_MAX_LEVEL; a++)
+            for (int L = 0; L < 8; L++) A.base[off][a][L] = hp->coef_base[off][a][L];
+        A.rec[off] = p->d_coef[off]; A.mom[off] = p->d_mom[off];
+    }
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) A.dV[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;
+}
+
+// Workspaces of the derivative variants (degree offsets 1, 2), allocated when first needed: collocation records
+// (with their static headers) and / or the moment vector.
+int need_workspace(gpw_plan *p, int off, bool coef, bool mom, cudaStream_t st, const char *who) {
+    const HostPlan *hp = p->hp;
+    const size_t nt = hp->task.size();
+    const size_t nw = (size_t)(hp->ncoef_total[off] ? hp->ncoef_total[off] : 1);
+    if (coef && !p->d_coef[off]) {
+        const size_t nrec = nw + 8 * nt;
+        if (!cuda_ok(cudaMalloc((void **)&p->d_coef[off], sizeof(double) * nrec), who)) return GPW_ENOMEM;
+        p->device_bytes += (long)(sizeof(double) * nrec);
+        if (!cuda_ok(cudaMemsetAsync(p->d_coef[off], 0, sizeof(double) * nrec, st), who)) return GPW_ECUDA;
+        if (nt) {
+            pp::PassArgs A;
+            fill_pass(p, A, 0);
+            k_rec_headers<<<((int)nt + 127) / 128, 128, 0, st>>>(p->d_taskK, p->d_taskP, (int)nt, A, off, p->d_coef[off]);
+            if (!cuda_ok(cudaGetLastError(), who)) return GPW_ECUDA;
+        }
+    }
+    if (mom && !p->d_mom[off]) {
+        if (!cuda_ok(cudaMalloc((void **)&p->d_mom[off], sizeof(double) * nw), who)) return GPW_ENOMEM;
+        p->device_bytes += (long)(sizeof(double) * nw);
+    }
+    return GPW_OK;
+}
 
 }  // namespace
 
@@ -231,21 +245,13 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
         for (int a = 0; a < hp->nlevel; a++) std::memcpy(S_all.data() + (size_t)a * S_TOTAL, hp->S[a].data(), sizeof(double) * S_TOTAL);
         ok = upload(&p->d_S, S_all.data(), S_all.size(), nb, "upload monomial maps");
     }
-    const size_t nw = (size_t)(hp->ncoef_total ? hp->ncoef_total : 1);
+    ok = ok && cuda_ok(cudaEventCreateWithFlags(&p->busy, cudaEventDisableTiming), "create event");
+    // collocation records [nP0 nP1 nP2 a_p c22 c23 c33 0 | polynomial] per pair (headers written once) and the
+    // moment workspace, for the degree offset 0; the derivative variants allocate theirs on first use
     if (ok) {
-        // collocation records: [nP0 nP1 nP2 a_p c22 c23 c33 0 | polynomial] per pair, headers written once
-        const size_t nrec = nw + 8 * hp->taskK.size();
-        ok = cuda_ok(cudaMalloc((void **)&p->d_coef, sizeof(double) * nrec), "allocate pair records") &&
-             cuda_ok(cudaMemsetAsync(p->d_coef, 0, sizeof(double) * nrec, 0), "clear pair records");
-        if (ok) {
-            nb += (long)(sizeof(double) * nrec);
-            const int nt = (int)hp->taskK.size();
-            if (nt) k_rec_headers<<<(nt + 127) / 128, 128>>>(p->d_taskK, nt, p->d_coef);
-            ok = cuda_ok(cudaGetLastError(), "pair record headers");
-        }
+        const int wrc = need_workspace(p, 0, true, true, 0, "allocate pair workspaces");
+        if (wrc != GPW_OK) { free_device(p); delete hp; delete p; return wrc; }
     }
-    ok = ok && cuda_ok(cudaMalloc((void **)&p->d_mom, sizeof(double) * nw), "allocate moment workspace");
-    if (ok) nb += (long)(sizeof(double) * nw);
     if (ok) {
         const size_t nvg = (size_t)hp->nvisit_total * visit_gauss_doubles(hp->ortho);
         ok = cuda_ok(cudaMalloc((void **)&p->d_vg, sizeof(double) * (nvg ? nvg : 1)), "allocate visit Gaussians");
@@ -275,7 +281,6 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
                  cuda_ok(cudaDeviceSynchronize(), "entry Gaussians");
         }
     }
-    ok = ok && cuda_ok(cudaEventCreateWithFlags(&p->busy, cudaEventDisableTiming), "create event");
     if (!ok) {
         free_device(p);
         delete hp;
@@ -308,7 +313,7 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
             for (int j = 0; j <= MAXL; j++) out->nvisit_class[a][i][j] = hp->nvisit_class[a][i][j];
     }
     out->nitem = hp->nitem;
-    out->ncoef_total = (long)hp->ncoef_total;
+    out->ncoef_total = (long)hp->ncoef_total[0];
     out->build_seconds = hp->build_seconds;
     out->device_bytes = p->device_bytes + interp_bytes(p->interp);
     return GPW_OK;
@@ -372,7 +377,7 @@ int gpw_plan_export_visits(const gpw_plan *p, gpw_visit *buf, long cap, long *nv
 
 int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *const *rho_dev, void *cuda_stream) {
     if (!p || !D_dev || !rho_dev) { set_error("gpw_eval_rho: null argument"); return GPW_EINVAL; }
-    if (deriv != 0 && deriv != 1) { set_error("gpw_eval_rho: deriv must be 0 or 1"); return GPW_EINVAL; }
+    if (deriv < 0 || deriv > 2) { set_error("gpw_eval_rho: deriv must be 0, 1 or 2"); return GPW_EINVAL; }
     if (!p->on_device) { set_error("gpw_eval_rho: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     const HostPlan *hp = p->hp;
     for (int a = 0; a < hp->nlevel; a++) {
@@ -381,7 +386,8 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (const int rc = begin_call(p, st, "gpw_eval_rho")) return rc;
-    const int ncomp = deriv ? 4 : 1;
+    gpw_plan *pm = const_cast<gpw_plan *>(p);
+    const int ncomp = deriv == 0 ? 1 : (deriv == 1 ? 4 : 5);
     for (int a = 0; a < hp->nlevel; a++) {
         const LevelGeom &g = hp->lev[a];
         const size_t nb = sizeof(double) * (size_t)g.N[0] * g.N[1] * g.N[2] * ncomp;
@@ -389,14 +395,23 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     }
     const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_rho");
-    gpw_plan *pm = const_cast<gpw_plan *>(p);
+    if (deriv == 2)
+        if (const int rc = need_workspace(pm, 2, true, false, st, "gpw_eval_rho: kinetic-energy workspace")) return rc;
     if (p->timing) { cudaEventRecord(p->ev[0][0], st); pm->ev_valid[0] = true; }
-    k_poly_from_D<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, D_dev, hp->nao, p->d_S, p->d_coef);
+    pp::PassArgs A;
+    fill_pass(p, A, pp::PRE_DENS | (deriv == 2 ? pp::PRE_TAU : 0));
+    A.D = D_dev;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_rho: pre-pass launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef, p->d_vg, deriv, hp->max_L, hp->ortho, st),
+    if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef[0], p->d_vg, deriv ? 1 : 0, 0, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
+    if (deriv == 2) {   // fifth component: tau, polynomials of degree L + 2, value only (Eq. 15)
+        fill_params(p, P, rho_dev, 2, 4);
+        if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef[2], p->d_vg, 0, 2, hp->max_L, hp->ortho, st),
+                     "gpw_eval_rho: kinetic-energy collocation launch")) return GPW_ECUDA;
+    }
     if (p->timing) cudaEventRecord(p->ev[0][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_rho: kernel launch")) return GPW_ECUDA;
     return end_call(p, st, "gpw_eval_rho");
@@ -404,7 +419,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
 
 int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, double *F_dev, void *cuda_stream) {
     if (!p || !v_dev || !F_dev) { set_error("gpw_eval_mat: null argument"); return GPW_EINVAL; }
-    if (deriv != 0 && deriv != 1) { set_error("gpw_eval_mat: deriv must be 0 or 1"); return GPW_EINVAL; }
+    if (deriv < 0 || deriv > 2) { set_error("gpw_eval_mat: deriv must be 0, 1 or 2"); return GPW_EINVAL; }
     if (!p->on_device) { set_error("gpw_eval_mat: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
     const HostPlan *hp = p->hp;
     for (int a = 0; a < hp->nlevel; a++) {
@@ -413,23 +428,59 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (const int rc = begin_call(p, st, "gpw_eval_mat")) return rc;
+    gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_mat");
-    if (!cuda_ok(cudaMemsetAsync(p->d_mom, 0, sizeof(double) * (size_t)hp->ncoef_total, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
+    if (deriv == 2)
+        if (const int rc = need_workspace(pm, 2, false, true, st, "gpw_eval_mat: kinetic-energy workspace")) return rc;
+    if (!cuda_ok(cudaMemsetAsync(p->d_mom[0], 0, sizeof(double) * (size_t)hp->ncoef_total[0], st), "gpw_eval_mat: memset")) return GPW_ECUDA;
+    if (deriv == 2 && !cuda_ok(cudaMemsetAsync(p->d_mom[2], 0, sizeof(double) * (size_t)hp->ncoef_total[2], st), "gpw_eval_mat: memset")) return GPW_ECUDA;
     GridParams P;
     fill_params(p, P, const_cast<double *const *>(v_dev));
-    gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (p->timing) { cudaEventRecord(p->ev[1][0], st); pm->ev_valid[1] = true; }
-    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, p->d_mom, deriv,
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, p->d_mom[0], deriv ? 1 : 0, 0,
                                   hp->max_L, hp->ortho, st), "gpw_eval_mat: integration launch")) return GPW_ECUDA;
+    if (deriv == 2) {   // fifth component: the kinetic-energy potential against 1/2 grad phi . grad phi (Eq. 16): moments to degree L + 2
+        fill_params(p, P, const_cast<double *const *>(v_dev), 2, 4);
+        if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, p->d_mom[2], 0, 2,
+                                      hp->max_L, hp->ortho, st), "gpw_eval_mat: kinetic-energy integration launch")) return GPW_ECUDA;
+    }
     if (p->timing) cudaEventRecord(p->ev[1][1], st);
-    DVs dv;
-    for (int a = 0; a < GPW_MAX_LEVEL; a++) dv.v[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;
-    k_F_from_moments<<<(ntask + 127) / 128, 128, 0, st>>>(p->d_taskP, ntask, p->d_mom, p->d_S, dv, F_dev, hp->nao);
+    pp::PassArgs A;
+    fill_pass(p, A, pp::POST_MAT | (deriv == 2 ? pp::POST_TAU : 0));
+    A.F = F_dev;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_mat: post-pass launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[1][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat: kernel launch")) return GPW_ECUDA;
     return end_call(p, st, "gpw_eval_mat");
+}
+
+int gpw_eval_grad(gpw_plan *p, const double *const *v_dev, int deriv, const double *D_dev, double *grad_dev, void *cuda_stream) {
+    if (!p || !v_dev || !D_dev || !grad_dev) { set_error("gpw_eval_grad: null argument"); return GPW_EINVAL; }
+    if (deriv != 0 && deriv != 1) { set_error("gpw_eval_grad: deriv must be 0 or 1"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_grad: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++) {
+        if (!v_dev[a]) { set_error("gpw_eval_grad: null level pointer"); return GPW_EINVAL; }
+        if (!aligned16(v_dev[a])) { set_error("gpw_eval_grad: level pointers must be 16-byte aligned"); return GPW_EINVAL; }
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, "gpw_eval_grad")) return rc;
+    if (!cuda_ok(cudaMemsetAsync(grad_dev, 0, sizeof(double) * 3 * (size_t)hp->natm, st), "gpw_eval_grad: memset")) return GPW_ECUDA;
+    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
+    if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_grad");
+    if (const int rc = need_workspace(p, 1, false, true, st, "gpw_eval_grad: workspace")) return rc;
+    if (!cuda_ok(cudaMemsetAsync(p->d_mom[1], 0, sizeof(double) * (size_t)hp->ncoef_total[1], st), "gpw_eval_grad: memset")) return GPW_ECUDA;
+    GridParams P;
+    fill_params(p, P, const_cast<double *const *>(v_dev), 1);
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, p->d_mom[1], deriv, 1,
+                                  hp->max_L, hp->ortho, st), "gpw_eval_grad: integration launch")) return GPW_ECUDA;
+    pp::PassArgs A;
+    fill_pass(p, A, pp::POST_GRAD);
+    A.D = D_dev; A.grad = grad_dev;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_grad: post-pass launch")) return GPW_ECUDA;
+    return end_call(p, st, "gpw_eval_grad");
 }
 
 int gpw_plan_set_timing(gpw_plan *p, int enable) {

@@ -18,6 +18,11 @@ namespace gpw {
 constexpr int MAXL = GPW_MAX_L;          // shells up to f
 constexpr int MAXLP = 2 * MAXL;          // pair polynomial degree L = la + lb <= 6
 constexpr int NLSEG = MAXLP + 1;         // visit lists are segmented by L = 0..6
+// Degree offsets: the grid kernels evaluate a pair polynomial (or accumulate pair moments) of degree L + off.
+//   off 0: density / potential (Eq. 3-4);  off 1: nuclear gradient (Alg. 3: one derivative of one function);
+//   off 2: kinetic-energy density tau and its potential (Eq. 15-16: one derivative of each function)
+constexpr int NOFF = 3;
+constexpr int MAXDEG = MAXLP + NOFF - 1; // largest polynomial degree, 8
 constexpr int TILE = 4;                  // grid block edge
 // integration stages bricks of BR1 x BR2 x BR3 grid blocks in shared memory; one block thick along n1 so
 // that a lane (which owns one n1 plane of a block) keeps the same u1 for every block of a brick entry
@@ -52,7 +57,7 @@ struct TaskK {
     double ap;           // a_p = a_a + a_b
     double c22, c23;     // exp(-2 a_p Gm22), exp(-2 a_p Gm23): second-order ratios of the Gaussian recursion
     double c33;          // exp(-2 a_p Gm33)   (Eq. 25; the cross term is the integer-index reading of A.31-A.32)
-    long long coef_off;  // offset (doubles) of the pair's polynomial / moment vector in the workspace
+    long long coef_off;  // offset (doubles) of the pair's polynomial / moment vector in the degree-L workspace
 };
 static_assert(sizeof(TaskK) == 64, "TaskK must be 64 bytes");
 
@@ -61,12 +66,14 @@ struct TaskP {
     double PA[3];    // P - A
     double PB[3];    // P - (B + T)
     double pref;     // coef_a coef_b exp(-a_a a_b / a_p |A - B - T|^2)
-    long long coef_off;
+    double aa, ab;   // the two primitive exponents (derivative variants: Eq. 15-16, Alg. 3)
     int ao_a, ao_b;
+    int atom_a, atom_b;
     short la, lb;
     short level;
     short sym;       // 1: use D_ab + D_ba and mirror F (hermi, not the a==b,T==0 pair)
 };
+static_assert(sizeof(TaskP) == 96, "TaskP must be 96 bytes");
 
 // One (pair, 4x4x4 block) visit in a block's list.
 struct Visit {
@@ -129,10 +136,10 @@ struct HostPlan {
     std::vector<HostTask> task;           // sorted by (level, L, enumeration order)
     std::vector<TaskK> taskK;
     std::vector<TaskP> taskP;
-    long long ncoef_total = 0;
-    // workspace offset of pair i of class (level, L) = coef_base[level][L] + i * ncoef_pad(L)
-    long long coef_base[GPW_MAX_LEVEL][NLSEG + 1] = {{0}};
-    bool coef_base_set[GPW_MAX_LEVEL][NLSEG + 1] = {{false}};
+    // per degree offset `off`: workspace offset of pair i (global index) of class (level, L)
+    //   = coef_base[off][level][L] + i * ncoef_pad(L + off);   ncoef_total[off] doubles in all
+    long long ncoef_total[NOFF] = {0};
+    long long coef_base[NOFF][GPW_MAX_LEVEL][NLSEG + 1] = {{{0}}};
     // per level block lists
     std::vector<std::vector<long long>> tile_base;   // [level][ntile+1] global visit index
     std::vector<std::vector<unsigned>> seg;          // [level][ntile*8] start of each L segment (relative)
@@ -147,6 +154,8 @@ struct HostPlan {
     double circ[GPW_MAX_LEVEL] = {0};                // circumradius of a 4x4x4 block about its centre, per level
     int max_L = 0;                                   // largest la + lb present
     bool ortho = false;                              // the lattice vectors are mutually orthogonal (every Gm diagonal)
+    bool hdiag = false;                              // ... and along the Cartesian axes (every H, hence every S_d, diagonal)
+    int max_l = 0;                                   // largest shell angular momentum
     long nvisit_level[GPW_MAX_LEVEL] = {0};
     long ntask_level[GPW_MAX_LEVEL] = {0};
     long nvisit_class[GPW_MAX_LEVEL][MAXL + 1][MAXL + 1] = {{{0}}};
@@ -159,7 +168,7 @@ GPW_CX int s_block_off(int d) {
     for (int e = 0; e < d; e++) { int n = (e + 1) * (e + 2) / 2; o += n * n; }
     return o;
 }
-constexpr int S_TOTAL = 1 + 9 + 36 + 100 + 225 + 441 + 784;
+constexpr int S_TOTAL = s_block_off(MAXDEG + 1);   // degree blocks 0..8: 4917 doubles
 
 void set_error(const std::string &msg);
 

@@ -13,23 +13,14 @@ struct GridParams {
     const unsigned *seg[GPW_MAX_LEVEL];          // collocation: per block, start of each L segment
     const long long *brick_base[GPW_MAX_LEVEL];  // integration: per brick, start of its entry list
     double *grid[GPW_MAX_LEVEL];                 // rho (written) or v (read)
-    long long coef_base[GPW_MAX_LEVEL][8];       // workspace offset of pair i of class (level, L) = base + i * ncoef_pad(L)
+    long long coef_base[GPW_MAX_LEVEL][8];       // workspace offset of pair i of class (level, L) = base + i * ncoef_pad(L + off),
+                                                 // off = the degree offset of the launch
 };
 
-// Pair record as the kernels use it, loaded with four 16-byte loads.
+// Pair record as the kernels use it.
 struct PairRec {
     double nP0, nP1, nP2, ap, c22, c23, c33;
-    long long coef_off;
 };
-
-__device__ __forceinline__ PairRec load_pair(const TaskK *__restrict__ tasks, int task) {
-    const double2 *tk = reinterpret_cast<const double2 *>(tasks + task);
-    const double2 a = __ldg(tk), b = __ldg(tk + 1), c = __ldg(tk + 2), d = __ldg(tk + 3);
-    PairRec r;
-    r.nP0 = a.x; r.nP1 = a.y; r.nP2 = b.x; r.ap = b.y; r.c22 = c.x; r.c23 = c.y; r.c33 = d.x;
-    r.coef_off = __double_as_longlong(d.y);
-    return r;
-}
 
 // cp.async helpers (records staged in shared memory ahead of their use)
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -48,18 +39,25 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // by the pair polynomial; the record of pair i of class (level, L) starts at coef_base[level][L] + i * (8 + ncoef_pad(L))
 // vg: Gaussian values of every visit (visit_gauss_doubles(ortho) per visit, order of `visits`), written once per
 // plan by launch_visit_gauss
+// off: degree offset of the launch (0, or 2 with deriv = 0: kinetic-energy density); rec and P.coef_base are those of `off`
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
-                             const double *rec, const double *vg, int deriv, int max_L, bool ortho, cudaStream_t st);
+                             const double *rec, const double *vg, int deriv, int off, int max_L, bool ortho, cudaStream_t st);
 size_t visit_gauss_doubles(bool ortho);
 cudaError_t launch_visit_gauss(const GridParams &P, int ntile_all, const TaskK *tasks, const Visit *visits, double *vg,
                                bool ortho, cudaStream_t st);
 // eg: 1-D Gaussian factor tables of every brick entry (entry_gauss_doubles(ortho) per entry, order of `entries`;
 // orthogonal cells only, else unused), written once per plan by launch_entry_gauss
+// off: degree offset (0; 1 with deriv 0 / 1: nuclear gradient; 2 with deriv = 0: kinetic-energy potential); the moments of
+// pair i of class (level, L) are added at mom + P.coef_base[level][L] + i * ncoef_pad(L + off)
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, const double *eg, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st);
+                             int nitem, const double *eg, double *mom, int deriv, int off, int max_L, bool ortho, cudaStream_t st);
 size_t entry_gauss_doubles(bool ortho);
 cudaError_t launch_entry_gauss(const GridParams &P, int nbrick_all, const TaskK *tasks, const BEntry *entries, double *eg,
                                cudaStream_t st);
+
+// pairpass.cu: pre- and post-pass (pairpass.cuh); max_l = the largest shell angular momentum of the plan
+namespace pp { struct PassArgs; }
+cudaError_t launch_pair_pass(const pp::PassArgs &A, int max_l, cudaStream_t st);
 
 // interp.cu: Eq. (7)-(8) with cuFFT; the state (plans, scratch) is created on first use; return a gpw_status
 struct InterpState;

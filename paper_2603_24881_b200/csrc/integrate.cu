@@ -57,12 +57,11 @@ struct BrickCtx {
 
 template <int L, int DERIV, bool ORTHO>
 __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, const double *prs, const double *gt,
-                                            bool valid, double *__restrict__ mom) {
+                                            bool valid, double *__restrict__ dst) {
     // the pair record (TaskK) staged in the group's shared-memory slot
     PairRec pr;
     pr.nP0 = prs[0]; pr.nP1 = prs[1]; pr.nP2 = prs[2]; pr.ap = prs[3];
     pr.c22 = prs[4]; pr.c23 = prs[5]; pr.c33 = prs[6];
-    pr.coef_off = __double_as_longlong(prs[7]);
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int CHS = chunk_doubles(NCOMP);
     constexpr int NB = npair2(L), NBX = npair2(L - 1);
@@ -122,7 +121,6 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
     pw1[0] = 1.0;
 #pragma unroll
     for (int k = 1; k <= L; k++) pw1[k] = pw1[k - 1] * u1;
-    double *dst = mom + pr.coef_off;
 #pragma unroll
     for (int kz = 0; kz <= L; kz++)
 #pragma unroll
@@ -137,10 +135,12 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
             }
 }
 
-template <int DERIV, int LMAX, bool ORTHO>
+// LMAX: largest la + lb held by the instantiation.  LOFF: degree offset -- the moments of a pair of class L are
+// accumulated up to degree L + LOFF (0: Eq. 4; 1: nuclear gradient, Alg. 3; 2: kinetic-energy potential, Eq. 16).
+template <int DERIV, int LMAX, bool ORTHO, int LOFF>
 // deriv = 0 with f shells (L up to 6): three CTAs per SM leave 168 registers and the L = 5, 6 bodies spill; two CTAs
 // at 220 registers without spills are faster (cfg3 k_integrate 2.40 -> 2.31 ms)
-__global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX > 4) ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
+__global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
                                                                           const TaskK *__restrict__ tasks,
                                                                           const BEntry *__restrict__ entries,
                                                                           const BItem *__restrict__ items,
@@ -294,14 +294,17 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX > 4) ? 2 : 3) k_int
         const double *gt = mygt + ps * EG;
         const bool valid = c0.base + grp < c0.hi;
         const BEntry enc = decode(e0);
+        // the pair's moment vector: class base + pair index * vector length (degree L + LOFF)
+        const int deg = c0.L + LOFF;
+        double *dst = mom + P.coef_base[level][c0.L] + (long long)enc.task * (((deg + 1) * (deg + 2) * (deg + 3) / 6 + 1) & ~1);
         switch (c0.L) {
-            case 0: integ_entry<0, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            case 1: integ_entry<1, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            case 2: integ_entry<2, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            case 5: if constexpr (LMAX >= 5) integ_entry<5, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
-            default: if constexpr (LMAX >= 6) integ_entry<6, DERIV, ORTHO>(c, enc, prs, gt, valid, mom); break;
+            case 0: integ_entry<0 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 1: integ_entry<1 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 2: integ_entry<2 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 3: if constexpr (LMAX >= 3) integ_entry<3 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 4: if constexpr (LMAX >= 4) integ_entry<4 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 5: if constexpr (LMAX >= 5) integ_entry<5 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            default: if constexpr (LMAX >= 6) integ_entry<6 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
         }
         c0 = c1; e0 = e1;
         c1 = c2; e1 = e2;
@@ -310,7 +313,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX > 4) ? 2 : 3) k_int
     cp_async_wait<0>();
 }
 
-template <int DERIV, int LMAX, bool ORTHO>
+template <int DERIV, int LMAX, bool ORTHO, int LOFF>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    const double *eg, double *mom, cudaStream_t st) {
     constexpr int smem = brick_doubles(DERIV ? 4 : 1, ORTHO) * (int)sizeof(double);
@@ -320,26 +323,44 @@ cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entrie
     if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
     const bool known = dev >= 0 && dev < 64;
     if (!known || !configured_dev[dev]) {
-        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO, LOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (known) configured_dev[dev] = true;
     }
-    k_integrate<DERIV, LMAX, ORTHO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
+    k_integrate<DERIV, LMAX, ORTHO, LOFF><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
     return cudaGetLastError();
 }
 
 template <int DERIV, bool ORTHO>
 cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                      const double *eg, double *mom, int max_L, cudaStream_t st) {
-    if (max_L <= 2) return launch<DERIV, 2, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
-    if (max_L <= 4) return launch<DERIV, 4, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
-    return launch<DERIV, 6, ORTHO>(P, tasks, entries, items, nitem, eg, mom, st);
+    if (max_L <= 2) return launch<DERIV, 2, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
+    return launch<DERIV, 6, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
+}
+// moments of degree L + LOFF (nuclear gradient: LOFF = 1, value or value + gradient field; kinetic-energy
+// potential: LOFF = 2, value only)
+template <int DERIV, bool ORTHO, int LOFF>
+cudaError_t launch_off(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
+                       const double *eg, double *mom, int max_L, cudaStream_t st) {
+    if (max_L <= 4) return launch<DERIV, 4, ORTHO, LOFF>(P, tasks, entries, items, nitem, eg, mom, st);
+    return launch<DERIV, 6, ORTHO, LOFF>(P, tasks, entries, items, nitem, eg, mom, st);
 }
 
 }  // namespace
 
 cudaError_t launch_integrate(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items,
-                             int nitem, const double *eg, double *mom, int deriv, int max_L, bool ortho, cudaStream_t st) {
+                             int nitem, const double *eg, double *mom, int deriv, int off, int max_L, bool ortho, cudaStream_t st) {
+    if (off == 2 && deriv == 0)
+        return ortho ? launch_off<0, true, 2>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
+                     : launch_off<0, false, 2>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
+    if (off == 1 && deriv == 0)
+        return ortho ? launch_off<0, true, 1>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
+                     : launch_off<0, false, 1>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
+    if (off == 1)
+        return ortho ? launch_off<1, true, 1>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
+                     : launch_off<1, false, 1>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
+    if (off != 0) return cudaErrorInvalidValue;
     if (deriv) return ortho ? launch_l<1, true>(P, tasks, entries, items, nitem, eg, mom, max_L, st)
                             : launch_l<1, false>(P, tasks, entries, items, nitem, eg, mom, max_L, st);
     return ortho ? launch_l<0, true>(P, tasks, entries, items, nitem, eg, mom, max_L, st)

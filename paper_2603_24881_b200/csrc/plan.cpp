@@ -71,21 +71,22 @@ inline int graded_idx(int a, int b, int d) {
 // S_d[row (p,q,r)][col (a,b,c)] = coefficient of u1^p u2^q u3^r in (H0.u)^a (H1.u)^b (H2.u)^c
 void build_S(const double *H, std::vector<double> &S) {
     S.assign(S_TOTAL, 0.0);
-    for (int d = 0; d <= MAXLP; d++) {
+    constexpr int ND = MAXDEG + 1;
+    for (int d = 0; d <= MAXDEG; d++) {
         const int nd = (d + 1) * (d + 2) / 2;
         double *blk = S.data() + s_block_off(d);
         for (int a = d; a >= 0; a--)
             for (int b = d - a; b >= 0; b--) {
                 const int c = d - a - b;
                 const int col = graded_idx(a, b, d);
-                double poly[MAXLP + 1][MAXLP + 1][MAXLP + 1];
+                double poly[ND][ND][ND];
                 std::memset(poly, 0, sizeof(poly));
                 poly[0][0][0] = 1.0;
                 int deg = 0;
                 const int reps[3] = {a, b, c};
                 for (int x = 0; x < 3; x++)
                     for (int rep = 0; rep < reps[x]; rep++) {
-                        double nxt[MAXLP + 1][MAXLP + 1][MAXLP + 1];
+                        double nxt[ND][ND][ND];
                         std::memset(nxt, 0, sizeof(nxt));
                         for (int p = 0; p <= deg; p++)
                             for (int q = 0; q <= deg - p; q++) {
@@ -222,6 +223,10 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         for (int a = 0; a < nlevel; a++)
             for (int k = 3; k < 6; k++)
                 if (hp->lev[a].Gm[k] != 0.0) hp->ortho = false;
+        hp->hdiag = true;
+        for (int i = 0; i < 9; i++)
+            if (i % 4 != 0 && cell[i] != 0.0) hp->hdiag = false;
+        for (int s = 0; s < nshl; s++) hp->max_l = std::max(hp->max_l, shl_l[s]);
 
         // circumradius of a block about its centre (points at +-1.5 steps per axis)
         for (int a = 0; a < nlevel; a++) {
@@ -326,10 +331,11 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         size_t nt = 0;
         for (auto &v : per_shell) nt += v.size();
         if (nt > 2000000000ull) { delete hp; set_error("gpw_build_pairs: more than 2^31 pairs"); return GPW_EUNSUPPORTED; }
-        // counting sort by class (level, L), keeping enumeration order inside a class: per shell the number of
-        // its pairs in every class, prefix sums over (class, shell), then every shell scatters its own pairs
-        constexpr int NCLS = GPW_MAX_LEVEL * 8;
-        auto cls_of = [](const HostTask &t) { return t.level * 8 + t.la + t.lb; };
+        // counting sort by class (level, L, la), keeping enumeration order inside a class: per shell the number of
+        // its pairs in every class, prefix sums over (class, shell), then every shell scatters its own pairs.
+        // (The kernels need (level, L); la inside keeps the lanes of the pre/post-pass on the same loop bounds.)
+        constexpr int NCLS = GPW_MAX_LEVEL * 8 * 4;
+        auto cls_of = [](const HostTask &t) { return (t.level * 8 + t.la + t.lb) * 4 + t.la; };
         std::vector<long> start((size_t)nshl * NCLS, 0);
         parallel_chunks(nshl, 16, nthread, [&](long, long lo, long hi, int) {
             for (long sa = lo; sa < hi; sa++)
@@ -358,15 +364,16 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         });
         const long ntask = (long)hp->task.size();
         hp->taskK.resize(ntask); hp->taskP.resize(ntask);
-        // inside a class the workspace offset is affine in the pair index: coef_base + i * ncoef_pad(L)
-        long long coff = 0;
-        for (int c = 0; c < NCLS; c++) {
-            const long n = cls_first[c + 1] - cls_first[c];
-            const int level = c / 8, L = c % 8;
+        // inside a class (level, L) the workspace offset is affine in the pair index: coef_base + i * ncoef_pad(L + off)
+        long long coff[NOFF] = {0};
+        for (int c = 0; c < NCLS; c += 4) {
+            const long n = cls_first[c + 4] - cls_first[c];
+            const int level = c / 32, L = (c / 4) % 8;
             if (n == 0 || L > MAXLP) continue;
-            hp->coef_base_set[level][L] = true;
-            hp->coef_base[level][L] = coff - (long long)cls_first[c] * ncoef_pad(L);
-            coff += (long long)n * ncoef_pad(L);
+            for (int off = 0; off < NOFF; off++) {
+                hp->coef_base[off][level][L] = coff[off] - (long long)cls_first[c] * ncoef_pad(L + off);
+                coff[off] += (long long)n * ncoef_pad(L + off);
+            }
             hp->ntask_level[level] += n;
             hp->max_L = std::max(hp->max_L, L);
         }
@@ -375,7 +382,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 const HostTask &t = hp->task[i];
                 const LevelGeom &g = hp->lev[t.level];
                 const int L = t.la + t.lb;
-                const long long off = hp->coef_base[t.level][L] + (long long)i * ncoef_pad(L);
+                const long long off = hp->coef_base[0][t.level][L] + (long long)i * ncoef_pad(L);
                 TaskK &k = hp->taskK[i];
                 for (int a = 0; a < 3; a++)
                     k.nP[a] = (t.P[0] * hp->binv[0 * 3 + a] + t.P[1] * hp->binv[1 * 3 + a] + t.P[2] * hp->binv[2 * 3 + a]) * g.N[a];
@@ -386,12 +393,14 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 k.coef_off = off;
                 TaskP &p = hp->taskP[i];
                 for (int x = 0; x < 3; x++) { p.PA[x] = t.P[x] - t.A[x]; p.PB[x] = t.P[x] - t.Bt[x]; }
-                p.pref = t.pref; p.coef_off = off;
+                p.pref = t.pref;
+                p.aa = prim_exp[t.prim_a]; p.ab = prim_exp[t.prim_b];
                 p.ao_a = hp->ao_loc[t.shl_a]; p.ao_b = hp->ao_loc[t.shl_b];
+                p.atom_a = shl_atom[t.shl_a]; p.atom_b = shl_atom[t.shl_b];
                 p.la = (short)t.la; p.lb = (short)t.lb; p.level = (short)t.level; p.sym = (short)t.sym;
             }
         });
-        hp->ncoef_total = coff;
+        for (int off = 0; off < NOFF; off++) hp->ncoef_total[off] = coff[off];
         if (!build_lists) {   // the block / brick lists are built on the device (plan_device.cu)
             hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
             *out = hp;

@@ -8,7 +8,7 @@ TOL = 1e-11   # north_star: relative, max-norm, on rho (per level and component)
 
 def gpu_rho(plan, D, deriv):
     import torch
-    nc = 4 if deriv else 1
+    nc = {0: 1, 1: 4, 2: 5}[int(deriv)]
     Dd = torch.as_tensor(np.ascontiguousarray(D), device="cuda")
     rho = [torch.full((nc,) + tuple(int(x) for x in m), float("nan"), dtype=torch.float64, device="cuda")
            for m in plan.mesh]
@@ -24,6 +24,16 @@ def gpu_mat(plan, v, deriv):
     gpw.gpw_eval_mat(plan, vd, deriv, F)
     torch.cuda.synchronize()
     return F.cpu().numpy()
+
+
+def gpu_grad(plan, v, deriv, D, natm):
+    import torch
+    vd = [torch.as_tensor(np.ascontiguousarray(x), device="cuda") for x in v]
+    Dd = torch.as_tensor(np.ascontiguousarray(D), device="cuda")
+    g = torch.full((natm, 3), float("nan"), dtype=torch.float64, device="cuda")
+    gpw.gpw_eval_grad(plan, vd, deriv, Dd, g)
+    torch.cuda.synchronize()
+    return g.cpu().numpy()
 
 
 def relmax(a, b):

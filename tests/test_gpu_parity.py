@@ -11,7 +11,7 @@ import oracle
 import paper_2603_24881_b200 as gpw
 from paper_2603_24881_b200 import inputs
 
-from gpu_util import TOL, check_rho, gpu_mat, gpu_rho, relmax, tile_mask_to_points
+from gpu_util import TOL, check_rho, gpu_grad, gpu_mat, gpu_rho, relmax, tile_mask_to_points
 
 pytestmark = pytest.mark.gpu
 
@@ -26,9 +26,10 @@ def _plan(inp, hermi=None):
 
 
 @pytest.mark.parametrize("kind", ["cubic", "triclinic", "ortho", "wrap", "contracted", "resolved"])
-@pytest.mark.parametrize("deriv", [0, 1])
+@pytest.mark.parametrize("deriv", [0, 1, 2])
 @pytest.mark.parametrize("hermi", [1, 0])
 def test_small_cells_full_parity(kind, deriv, hermi):
+    """deriv = 2: the fifth component is tau (Eq. 15) / the v_tau term of F (Eq. 16), SURVEY 8(f) item 2."""
     inp = inputs.make_small(kind, deriv=deriv, hermi=hermi)
     o = oracle.Oracle.from_inputs(inp)
     plan = _plan(inp)
@@ -40,6 +41,55 @@ def test_small_cells_full_parity(kind, deriv, hermi):
     F, Fo = gpu_mat(plan, v, deriv), o.eval_mat(v, deriv)
     assert np.isfinite(F).all()
     assert relmax(F, Fo) <= TOL
+
+
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "ortho", "wrap", "contracted", "resolved"])
+@pytest.mark.parametrize("deriv", [0, 1])
+@pytest.mark.parametrize("hermi", [1, 0])
+def test_small_cells_nuclear_gradient(kind, deriv, hermi):
+    """gpw_eval_grad (Alg. 3) against the oracle's orc_eval_grad: relative to the largest component."""
+    inp = inputs.make_small(kind, deriv=deriv, hermi=hermi)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    if not hermi:
+        D = D + 0.2 * np.random.default_rng(3).standard_normal(D.shape)
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    g = gpu_grad(plan, v, deriv, D, inp.natm)
+    go = o.eval_grad(v, deriv, D)
+    assert np.isfinite(g).all()
+    assert relmax(g, go) <= TOL
+    # the calls of the other kinds on the same plan are not disturbed by the gradient's workspace
+    assert relmax(gpu_mat(plan, v, deriv), o.eval_mat(v, deriv)) <= TOL
+
+
+def test_config1_meta_gga_and_gradient_sampled():
+    """cfg 1 (32 waters) with deriv = 2 on a sample of blocks / shell pairs, and the nuclear gradient in full."""
+    inp = dataclasses.replace(inputs.make_config(1), deriv=2)
+    o = oracle.Oracle.from_inputs(inp)
+    plan = _plan(inp)
+    D = inp.D()
+    rng = np.random.default_rng(11)
+    masks = [(rng.random(int(np.prod(m // 4))) < 0.05).astype(np.uint8) for m in inp.mesh]
+    ro = o.eval_rho(D, 2, tile_masks=masks)
+    rg = gpu_rho(plan, D, 2)
+    for lev in range(inp.nlevel):
+        pm = tile_mask_to_points(masks[lev], inp.mesh[lev])
+        for c in range(5):
+            den = np.abs(rg[lev][c]).max()
+            if den > 0:
+                assert np.abs(rg[lev][c][pm] - ro[lev][c][pm]).max() / den <= TOL
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    pmask = (rng.random((inp.nshl, inp.nshl)) < 0.05).astype(np.uint8)
+    Fo = o.eval_mat(v, 2, pair_mask=pmask)
+    F = gpu_mat(plan, v, 2)
+    ao = np.concatenate([[0], np.cumsum([(l + 1) * (l + 2) // 2 for l in inp.shl_l])])
+    sel = np.zeros((inp.nao, inp.nao), bool)
+    for a, b in zip(*np.nonzero(pmask)):
+        sel[ao[a]:ao[a + 1], ao[b]:ao[b + 1]] = True
+    assert np.abs(F[sel] - Fo[sel]).max() / np.abs(F).max() <= TOL
+    v1 = [x[:4] for x in v]
+    assert relmax(gpu_grad(plan, v1, 1, D, inp.natm), o.eval_grad(v1, 1, D)) <= TOL
 
 
 def test_hermi_uses_both_triangles_of_D():
