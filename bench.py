@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the multigrid GPW collocation + integration hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--deriv d] [--tau t] [--rel-cutoff c] [--impl reference]
 
 A step is one pass of the hot path on one synthetic workload: gpw_eval_rho on every level followed by
 gpw_eval_mat (the plan of gpw_build_pairs is built once beforehand; setup time is reported, not timed
@@ -72,12 +72,26 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows)}
 
 
+def csrc_sha() -> str:
+    """Hash of the kernel sources: ties the committed ncu figures (profiles/traffic.json) to the build they were taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2603_24881_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h", ".cpp")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def model_flops_from_counts(counts, deriv: int) -> float:
     nc = [1, 3, 6, 10]
     tot = 0.0
     for la in range(4):
         for lb in range(4):
-            w = (4 * nc[la] * nc[lb] + 10 * (nc[la] + nc[lb]) + 8) if deriv else (2 * nc[la] * nc[lb] + 2 * (nc[la] + nc[lb]) + 4)
+            w0 = 2 * nc[la] * nc[lb] + 2 * (nc[la] + nc[lb]) + 4
+            w1 = 4 * nc[la] * nc[lb] + 10 * (nc[la] + nc[lb]) + 8
+            w = (w0, w1, w1 + w0)[int(deriv)]   # deriv = 2: the tau contraction counted as one more value-like contraction
             tot += 64.0 * float(counts[:, la, lb].sum()) * w
     return tot
 
@@ -164,6 +178,10 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (default 2: 256 waters, GGA)")
+    ap.add_argument("--deriv", type=int, default=None, choices=[0, 1, 2],
+                    help="override the config's derivative level (2 = meta-GGA: a fifth component, tau / v_tau)")
+    ap.add_argument("--tau", type=float, default=None, help="override the screening threshold of Eq. 20 (configs: 1e-10; the paper used 1e-6)")
+    ap.add_argument("--rel-cutoff", type=float, default=None, help="override the level-assignment constant (configs: 20; reading A6)")
     ap.add_argument("--impl", default="gpw", choices=["gpw", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -172,10 +190,19 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
+    import dataclasses
     from paper_2603_24881_b200 import inputs
+
+    def workload(seed=None):
+        inp = inputs.make_config(args.config, seed=seed)
+        over = {k: v for k, v in (("deriv", args.deriv), ("tau", args.tau), ("rel_cutoff", args.rel_cutoff)) if v is not None}
+        if over:
+            inp = dataclasses.replace(inp, name=inp.name + "".join(f"+{k}={v:g}" for k, v in over.items()), **over)
+        return inp
+
     if args.impl == "reference":
         if rank == 0:
-            run_reference(args, inputs.make_config(args.config))
+            run_reference(args, workload())
         return
 
     import torch
@@ -189,7 +216,7 @@ def main():
     W = max(3, args.warmup)
 
     # every rank its own independent workload of the same shape (weak scaling)
-    inp = inputs.make_config(args.config, seed=rank_seed(args.config, rank))
+    inp = workload(rank_seed(args.config, rank))
     deriv, nc = inp.deriv, inp.ncomp
     t0 = time.time()
     plan = gpw.gpw_build_pairs(*inp.abi_args())
@@ -211,7 +238,6 @@ def main():
     resident_bytes = 2 * grid_bytes + 2 * inp.nao * inp.nao * 8
 
     peak_meas, nsm = gpw.gpw_dfma_peak(0.5)
-    gpw.gpw_plan_set_timing(plan, True)
 
     def step():
         gpw.gpw_eval_rho(plan, D, deriv, rho)
@@ -229,24 +255,32 @@ def main():
     time.sleep(0.3)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    kt = np.zeros(4)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     tw0 = time.time()
     e0.record()
-    for _ in range(args.steps):
+    marks[0].record()
+    for i in range(args.steps):   # nothing but the K steps (and one event record each) between the two brackets
         step()
-        # kernel durations from the library's own events on the launching stream (no extra sync: the
-        # query below waits only for this step, which the next step's launches would wait for anyway)
-        a = gpw.gpw_plan_get_timing(plan, 0)
-        b = gpw.gpw_plan_get_timing(plan, 1)
-        kt += np.array([a[0], a[1], b[0], b[1]])
+        marks[i + 1].record()
     e1.record()
     barrier()
     tw1 = time.time()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.summary(tw0, tw1)
     sampler.stop()
-    kt /= args.steps
+    per_step = np.array([marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps)])
     ms_step = ms_total / args.steps
+    # kernel durations from the library's own events on the launching stream, outside the timed region
+    gpw.gpw_plan_set_timing(plan, True)
+    kts = []
+    for _ in range(max(3, min(args.steps, 10))):
+        step()
+        a = gpw.gpw_plan_get_timing(plan, 0)
+        b = gpw.gpw_plan_get_timing(plan, 1)
+        kts.append([a[0], a[1], b[0], b[1]])
+    gpw.gpw_plan_set_timing(plan, False)
+    kt = np.median(np.array(kts), axis=0)
+    kt_min = np.min(np.array(kts), axis=0)
     ms_step, flops_all = reduce_over_ranks(ms_step, flops_step, dist, "cuda")
     value = flops_all / (ms_step * 1e-3) / 1e9
 
@@ -263,10 +297,13 @@ def main():
     rho_fine = torch.empty(fine_shape, dtype=torch.float64, device="cuda")
     v_fine = torch.randn(fine_shape, dtype=torch.float64, device="cuda", generator=gen)
     v_lev = [torch.empty(s, dtype=torch.float64, device="cuda") for s in shapes]
+    v_hartree = torch.empty(fine_shape[1:], dtype=torch.float64, device="cuda")
 
     def fock_step():
         gpw.gpw_eval_rho(plan, D, deriv, rho)
         gpw.gpw_interp_up(plan, rho, nc, rho_fine)
+        gpw.gpw_hartree(plan, rho_fine[0], v_hartree)     # Eq. 5-6: the Hartree potential of the collocated density
+        v_fine[0].copy_(v_hartree)                        # components 1.. (the XC side) stay synthetic
         gpw.gpw_restrict_down(plan, v_fine, nc, v_lev)
         gpw.gpw_eval_mat(plan, v_lev, deriv, F)
 
@@ -279,7 +316,7 @@ def main():
     e1.record()
     barrier()
     fock_ms = e0.elapsed_time(e1) / fock_steps
-    del rho_fine, v_fine, v_lev
+    del rho_fine, v_fine, v_lev, v_hartree
 
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----
     Dh = D.cpu().pin_memory()
@@ -289,24 +326,26 @@ def main():
     h2d = Dh.numel() * 8 + grid_bytes
     d2h = grid_bytes + Fh.numel() * 8
 
+    # the library's host-buffer entry points (include/gpw.h): every array in pinned host memory, uploads, kernels and
+    # downloads inside the timed region, overlapped by the library on its own copy streams
     def e2e_step():
-        D.copy_(Dh, non_blocking=True)
-        gpw.gpw_eval_rho(plan, D, deriv, rho)
-        for a, b in zip(rho_h, rho):
-            a.copy_(b, non_blocking=True)
-        for a, b in zip(v, vh):
-            a.copy_(b, non_blocking=True)
-        gpw.gpw_eval_mat(plan, v, deriv, F)
-        Fh.copy_(F, non_blocking=True)
+        gpw.gpw_eval_rho_host(plan, Dh, deriv, rho_h)
+        gpw.gpw_eval_mat_host(plan, vh, deriv, Fh)
 
     e2e_steps = max(2, min(args.steps, 5))
     e2e_step()
+    gpw.gpw_plan_wait(plan)
     barrier()
     e0.record()
     for _ in range(e2e_steps):
         e2e_step()
+    gpw.gpw_plan_wait(plan)      # the timing stream waits for the last download
     e1.record()
     barrier()
+    step()
+    barrier()
+    e2e_check = float((Fh - F.cpu()).abs().max() / F.abs().max())   # same result as the resident path
+    assert e2e_check <= 1e-12, e2e_check
     e2e_ms = e0.elapsed_time(e1) / e2e_steps
     e2e_ms, _ = reduce_over_ranks(e2e_ms, flops_step, dist, "cuda")
     e2e_value = flops_all / (e2e_ms * 1e-3) / 1e9
@@ -319,49 +358,67 @@ def main():
     # dominant kernel = the slower of collocation / integration
     dom = "k_integrate" if kt[2] >= kt[1] else "k_collocate"
     dom_ms = float(max(kt[1], kt[2]))
-    achieved = flops_call / (dom_ms * 1e-3) / 1e12
-    # DRAM bytes per launch, FP64-pipe utilisation and executed FP64 flops per launch of that kernel from the
-    # committed ncu capture of the same build (profiles/traffic.json names the capture), else null
-    traffic, ncu = None, {}
+    model_tflops = flops_call / (dom_ms * 1e-3) / 1e12
+    # Executed FP64 flops per launch (ncu: 2 DFMA + DADD + DMUL thread instructions), FP64-pipe utilisation and DRAM
+    # bytes per launch come from the committed full ncu capture of THIS build (profiles/traffic.json carries the hash
+    # of csrc/ it was taken on): a profiler cannot run inside a timed bench.  If the sources changed since, null.
+    sha = csrc_sha()
+    ncu, ncu_all = {}, {}
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
-            ncu = json.load(open(tpath)).get(f"{inp.name}:{dom}") or {}
-            traffic = ncu.get("dram_bytes")
+            tj = json.load(open(tpath))
+            if tj.get("csrc_sha") == sha:
+                ncu_all = tj.get("kernels", {})
+                ncu = ncu_all.get(f"{inp.name}:{dom}") or {}
         except Exception:
-            traffic, ncu = None, {}
+            ncu, ncu_all = {}, {}
     executed = ncu.get("executed_fp64_flops")
+    executed_tflops = (executed / (dom_ms * 1e-3) / 1e12) if executed else None
+
+    def exec_frac(kernel, ms):
+        e = (ncu_all.get(f"{inp.name}:{kernel}") or {}).get("executed_fp64_flops")
+        return (e / (ms * 1e-3) / 1e12 / NOMINAL_FP64_TFLOPS) if e else None
+
+    nlaunch = 4 + (2 if deriv == 2 else 0)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per_step)), "ms_per_step_min": float(per_step.min()),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": inp.name, "nao": inp.nao, "meshes": [int(m[0]) for m in inp.mesh], "deriv": deriv,
                    "tau": inp.tau, "rel_cutoff": inp.rel_cutoff, "hermi": inp.hermi,
                    "pairs": info["ntask"], "block_visits": int(sum(info["nvisit_level"])),
                    "l2": f"inputs+outputs resident {resident_bytes / 1e6:.0f} MB > 126 MB L2, no explicit flush",
-                   "flop_model": "SURVEY 8(d): 64*visits*W, W1=4*nca*ncb+10*(nca+ncb)+8 (deriv=1), W0=2*nca*ncb+2*(nca+ncb)+4"},
+                   "flop_model": "SURVEY 8(d): 64*visits*W, W1=4*nca*ncb+10*(nca+ncb)+8 (deriv>=1), W0=2*nca*ncb+2*(nca+ncb)+4; deriv=2: W1+W0"},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h)},
-        "gpu_launches": 4 * args.steps,
-        "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": NOMINAL_FP64_TFLOPS,
-                     "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP64_TFLOPS, "traffic": traffic,
+                "d2h_bytes_per_step": int(d2h),
+                "api": "gpw_eval_rho_host + gpw_eval_mat_host (C ABI, pinned host buffers; copies overlapped on the library's streams)"},
+        "gpu_launches": nlaunch * args.steps,
+        "roofline": {"bound": "alu", "kernel": dom, "achieved": executed_tflops, "peak": NOMINAL_FP64_TFLOPS,
+                     "unit": "TFLOP/s", "frac": (executed_tflops / NOMINAL_FP64_TFLOPS) if executed_tflops else None,
+                     "traffic": ncu.get("dram_bytes"),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
-                     "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
-                     "executed_tflops": (executed / (dom_ms * 1e-3) / 1e12) if executed else None,
-                     "executed_frac": (executed / (dom_ms * 1e-3) / 1e12 / NOMINAL_FP64_TFLOPS) if executed else None,
-                     "fp64_pipe_pct_ncu": ncu.get("fp64_pipe_pct"), "ncu_capture": ncu.get("capture"),
-                     "note": "achieved = model flops of one call / kernel time; the kernels evaluate a cheaper "
-                             "polynomial form, so executed FP64 flops (executed_tflops: ncu's 2*DFMA+DADD+DMUL "
-                             "thread instructions per launch / this run's kernel time) are lower than the model's (DESIGN.md)"},
-        "kernels_ms": {"k_poly_from_D": float(kt[0]), "k_collocate": float(kt[1]), "k_integrate": float(kt[2]),
-                       "k_F_from_moments": float(kt[3])},
+                     "peak_measured_dfma": peak_meas,
+                     "fp64_pipe_pct_ncu": ncu.get("fp64_pipe_pct"), "ncu_capture": ncu.get("capture"), "csrc_sha": sha,
+                     "frac_k_collocate": exec_frac("k_collocate", float(kt[1])), "frac_k_integrate": exec_frac("k_integrate", float(kt[2])),
+                     "model_tflops": model_tflops,
+                     "note": "achieved = FP64 flops the kernel EXECUTES per launch (ncu: 2*DFMA + DADD + DMUL thread instructions, "
+                             "from the committed capture of this very build, matched by csrc_sha; null if the sources changed since) "
+                             "/ this run's kernel time (CUDA events).  model_tflops = SURVEY 8(d) model flops of one call / the same "
+                             "time: the kernels evaluate a cheaper polynomial form than the model charges, so it can exceed the peak "
+                             "and is not a roofline fraction (DESIGN.md section 5)"},
+        "kernels_ms": {"k_pair_pass_pre": float(kt[0]), "k_collocate": float(kt[1]), "k_integrate": float(kt[2]),
+                       "k_pair_pass_post": float(kt[3])},
+        "kernels_ms_min": {"k_pair_pass_pre": float(kt_min[0]), "k_collocate": float(kt_min[1]), "k_integrate": float(kt_min[2]),
+                           "k_pair_pass_post": float(kt_min[3])},
         "model_gflop_per_call": flops_call / 1e9,
         "eval_rho_tflops_model": flops_call / ((kt[0] + kt[1]) * 1e-3) / 1e12,
         "eval_mat_tflops_model": flops_call / ((kt[2] + kt[3]) * 1e-3) / 1e12,
         "fock_build_ms": fock_ms,
-        "fock_build_note": "eval_rho + gpw_interp_up + gpw_restrict_down of a synthetic fine-grid N(0,1) field + eval_mat; "
-                           "XC and Hartree excluded",
+        "fock_build_note": "eval_rho + gpw_interp_up + gpw_hartree (Eq. 5-6) of the interpolated density + gpw_restrict_down of "
+                           "[v_H, synthetic N(0,1) XC-side components] + eval_mat; XC functional itself excluded (LibXC)",
         "plan_build_s": build_s, "plan_device_bytes": int(info["device_bytes"]),
         "adjointness_rel_err": adj,
     }

@@ -162,6 +162,23 @@ int gpw_eval_mat(const gpw_plan *plan, const double *const *v_dev, int deriv, do
                  void *cuda_stream);
 
 /*
+ * Host-buffer variants: the same two operations with every array in HOST memory (D_host [nao][nao]; rho_host /
+ * v_host: HOST arrays of nlevel HOST pointers [ncomp][N1][N2][N3]; F_host [nao][nao]).  The library uploads the
+ * inputs into staging buffers it owns, runs the kernels and downloads the results, on three streams of its own
+ * (upload, kernels, download) so that the copies of one call overlap the kernels and the opposite copies of its
+ * neighbours: an upload never waits for a download.  Pinned host memory (cudaHostAlloc / cudaHostRegister) is
+ * needed for that overlap; pageable memory works but serialises.
+ * Ordering: a call starts after the work already queued on cuda_stream; its OUTPUTS ARE COMPLETE only after
+ * gpw_plan_wait(plan, s) has been passed on a stream s (or the device has been synchronised) -- the caller's stream
+ * is not made to wait at the end of the call, so that successive calls pipeline.  Input buffers may be reused
+ * after the same point.  First use allocates the staging buffers (gpw_info.device_bytes).
+ */
+int gpw_eval_rho_host(gpw_plan *plan, const double *D_host, int deriv, double *const *rho_host, void *cuda_stream);
+int gpw_eval_mat_host(gpw_plan *plan, const double *const *v_host, int deriv, double *F_host, void *cuda_stream);
+/* Makes cuda_stream wait for every host-buffer call issued so far on the plan (their downloads included). */
+int gpw_plan_wait(gpw_plan *plan, void *cuda_stream);
+
+/*
  * Nuclear gradient (Alg. 3) of the grid energy
  *     E = sum_alpha dV_alpha sum_r [ v0(r) rho_alpha(r) + w(r) . grad rho_alpha(r) ]
  * at FIXED v0, w and fixed visit set, rho_alpha being the collocated density of gpw_eval_rho:
@@ -185,6 +202,19 @@ int gpw_interp_up(gpw_plan *plan, const double *const *rho_dev, int ncomp, doubl
                   void *cuda_stream);
 int gpw_restrict_down(gpw_plan *plan, const double *v_fine_dev, int ncomp, double *const *v_dev,
                       void *cuda_stream);
+
+/*
+ * G-space operators of the Fock build on the FINEST mesh (cuFFT + one pointwise kernel each; off target):
+ *   gpw_hartree            v_H(r) = sum_{G != 0} 4 pi / |G|^2 F(rho)(G) exp(i G . r)      Eq. (5)-(6)
+ *   gpw_gspace_gradient    grad rho (r) = sum_G i G F(rho)(G) exp(i G . r)                Eq. (10)
+ *   gpw_gspace_divergence  div w (r) = sum_G i G . F(w)(G) exp(i G . r)                   Eq. (14)
+ * G_m = 2 pi sum_i m_i b_i, b_i = i-th column of inverse(cell); plane waves on a Nyquist plane |m_i| = N_i / 2 are
+ * dropped (A26).  All pointers DEVICE, 16-byte aligned, on the level-0 mesh: rho / v_H / div [N1][N2][N3],
+ * grad / w [3][N1][N2][N3]; outputs OVERWRITTEN; in and out must not overlap.
+ */
+int gpw_hartree(gpw_plan *plan, const double *rho_fine_dev, double *vh_fine_dev, void *cuda_stream);
+int gpw_gspace_gradient(gpw_plan *plan, const double *rho_fine_dev, double *grad_fine_dev, void *cuda_stream);
+int gpw_gspace_divergence(gpw_plan *plan, const double *w_fine_dev, double *div_fine_dev, void *cuda_stream);
 
 /* Introspection (host). */
 int gpw_plan_info(const gpw_plan *plan, gpw_info *out);

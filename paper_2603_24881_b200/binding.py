@@ -57,6 +57,8 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _lib = None
 
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_eval_grad", "gpw_interp_up", "gpw_restrict_down",
+           "gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence",
+           "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait",
            "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
@@ -91,6 +93,15 @@ def load_library():
     L.gpw_restrict_down.restype = ctypes.c_int
     L.gpw_restrict_down.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_void_p), ctypes.c_void_p]
+    L.gpw_eval_rho_host.restype = ctypes.c_int
+    L.gpw_eval_rho_host.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_void_p), ctypes.c_void_p]
+    L.gpw_eval_mat_host.restype = ctypes.c_int
+    L.gpw_eval_mat_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    L.gpw_plan_wait.restype = ctypes.c_int
+    L.gpw_plan_wait.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+    for name in ("gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence"):
+        getattr(L, name).restype = ctypes.c_int
+        getattr(L, name).argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
     L.gpw_plan_info.restype = ctypes.c_int
     L.gpw_plan_info.argtypes = [ctypes.c_void_p, ctypes.POINTER(gpw_info)]
     L.gpw_plan_export_tasks.restype = ctypes.c_int
@@ -228,6 +239,37 @@ def gpw_eval_mat(plan: Plan, v: Sequence, deriv: int, F, stream=None):
     _check(load_library().gpw_eval_mat(plan._h, ptrs, int(deriv), ctypes.c_void_p(F.data_ptr()), _stream_ptr(stream)))
 
 
+def _check_host(t, shape, what):
+    import torch
+    if not (not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
+        raise ValueError(f"{what}: need a contiguous host float64 tensor of shape {shape}, got {tuple(t.shape)} {t.dtype} {t.device}")
+
+
+def gpw_eval_rho_host(plan: Plan, D, deriv: int, rho: Sequence, stream=None):
+    """Host-buffer variant: D and rho[level] are HOST tensors (pinned for overlap); complete after gpw_plan_wait."""
+    nc = NCOMP[int(deriv)]
+    _check_host(D, (plan.nao, plan.nao), "D")
+    for lev in range(plan.nlevel):
+        _check_host(rho[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"rho[{lev}]")
+    ptrs = (ctypes.c_void_p * plan.nlevel)(*[r.data_ptr() for r in rho])
+    _check(load_library().gpw_eval_rho_host(plan._h, ctypes.c_void_p(D.data_ptr()), int(deriv), ptrs, _stream_ptr(stream)))
+
+
+def gpw_eval_mat_host(plan: Plan, v: Sequence, deriv: int, F, stream=None):
+    """Host-buffer variant: v[level] and F are HOST tensors (pinned for overlap); complete after gpw_plan_wait."""
+    nc = NCOMP[int(deriv)]
+    _check_host(F, (plan.nao, plan.nao), "F")
+    for lev in range(plan.nlevel):
+        _check_host(v[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
+    ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
+    _check(load_library().gpw_eval_mat_host(plan._h, ptrs, int(deriv), ctypes.c_void_p(F.data_ptr()), _stream_ptr(stream)))
+
+
+def gpw_plan_wait(plan: Plan, stream=None):
+    """Make the stream wait for every host-buffer call issued so far on the plan."""
+    _check(load_library().gpw_plan_wait(plan._h, _stream_ptr(stream)))
+
+
 def gpw_eval_grad(plan: Plan, v: Sequence, deriv: int, D, grad, stream=None):
     """grad (CUDA float64 [natm, 3]) is overwritten with dE/dR of E = sum dV [v0 rho + w . grad rho] at fixed v, w."""
     nc = NCOMP[int(deriv)]
@@ -255,6 +297,28 @@ def gpw_restrict_down(plan: Plan, v_fine, ncomp: int, v: Sequence, stream=None):
     _check_grid(v_fine, (int(ncomp),) + tuple(int(x) for x in plan.mesh[0]), "v_fine")
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
     _check(load_library().gpw_restrict_down(plan._h, ctypes.c_void_p(v_fine.data_ptr()), int(ncomp), ptrs, _stream_ptr(stream)))
+
+
+def _gspace(name, plan, x, xshape, y, yshape, stream):
+    m = tuple(int(v) for v in plan.mesh[0])
+    _check_grid(x, xshape + m, "input")
+    _check_grid(y, yshape + m, "output")
+    _check(getattr(load_library(), name)(plan._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(y.data_ptr()), _stream_ptr(stream)))
+
+
+def gpw_hartree(plan: Plan, rho_fine, vh_fine, stream=None):
+    """vh_fine [N1, N2, N3] is overwritten with the Hartree potential of rho_fine (Eq. 5-6), both on the finest mesh."""
+    _gspace("gpw_hartree", plan, rho_fine, (), vh_fine, (), stream)
+
+
+def gpw_gspace_gradient(plan: Plan, rho_fine, grad_fine, stream=None):
+    """grad_fine [3, N1, N2, N3] is overwritten with the Fourier gradient of rho_fine (Eq. 10)."""
+    _gspace("gpw_gspace_gradient", plan, rho_fine, (), grad_fine, (3,), stream)
+
+
+def gpw_gspace_divergence(plan: Plan, w_fine, div_fine, stream=None):
+    """div_fine [N1, N2, N3] is overwritten with the Fourier divergence of w_fine [3, N1, N2, N3] (Eq. 14)."""
+    _gspace("gpw_gspace_divergence", plan, w_fine, (3,), div_fine, (), stream)
 
 
 def gpw_plan_set_timing(plan: Plan, enable: bool):
@@ -286,9 +350,7 @@ def model_flops(info: dict, deriv: int) -> float:
     for la in range(4):
         for lb in range(4):
             n = float(cls[:, la, lb].sum())
-            if deriv:
-                w = 4 * nc[la] * nc[lb] + 10 * (nc[la] + nc[lb]) + 8
-            else:
-                w = 2 * nc[la] * nc[lb] + 2 * (nc[la] + nc[lb]) + 4
-            total += 64.0 * n * w
+            w0 = 2 * nc[la] * nc[lb] + 2 * (nc[la] + nc[lb]) + 4
+            w1 = 4 * nc[la] * nc[lb] + 10 * (nc[la] + nc[lb]) + 8
+            total += 64.0 * n * (w0, w1, w1 + w0)[int(deriv)]   # deriv = 2: the tau contraction counted as one more W0
     return total

@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpw.so")
-SOURCES = ["plan.cpp", "plan_device.cu", "gpw_api.cu", "pairpass.cu", "collocate.cu", "integrate.cu", "interp.cu"]
-HEADERS = ["gpw_internal.h", "gpw_math.cuh", "gpw_kernels.cuh", "pairpass.cuh", "plan_device.h"]
+SOURCES = ["plan.cpp", "plan_device.cu", "gpw_api.cu", "pairpass.cu", "pairpass_reg_pre.cu", "pairpass_reg_post.cu", "collocate.cu", "integrate.cu", "interp.cu"]
+HEADERS = ["gpw_internal.h", "gpw_math.cuh", "gpw_kernels.cuh", "pairpass.cuh", "pairpass_reg.cuh", "pairpass_reg_kernel.cuh", "plan_device.h"]
 # plan_device.cu repeats the host builder's geometric block test: no FMA contraction, so that the two agree bit for bit
 EXTRA = {"plan_device.cu": ["-fmad=false"]}
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -42,19 +42,26 @@ def build(force: bool = False, verbose: bool = False) -> str:
         try:
             if not force and not _stale():
                 return LIB
-            return _build_locked(verbose)
+            return _build_locked(verbose, force)
         finally:
             fcntl.flock(lock, fcntl.LOCK_UN)
 
 
-def _build_locked(verbose: bool) -> str:
+def _build_locked(verbose: bool, force: bool = False) -> str:
+    """Compile what is out of date (an object is rebuilt when its source, any header or this file is newer), in
+    parallel, then link."""
+    hdrs = [os.path.join(CSRC, f) for f in HEADERS] + [os.path.join(ROOT, "include", "gpw.h"), os.path.abspath(__file__)]
+    hdr_t = max(os.path.getmtime(h) for h in hdrs)
     objs = []
     procs = []
     for src in SOURCES:
         obj = os.path.join(CSRC, os.path.splitext(src)[0] + ".o")
-        cmd = [NVCC] + FLAGS + EXTRA.get(src, []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
-        procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(obj)
+        path = os.path.join(CSRC, src)
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) > max(hdr_t, os.path.getmtime(path)):
+            continue
+        cmd = [NVCC] + FLAGS + EXTRA.get(src, []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", path, "-o", obj]
+        procs.append((cmd, subprocess.Popen(cmd)))
     for cmd, p in procs:
         if p.wait() != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))

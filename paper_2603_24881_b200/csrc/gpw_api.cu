@@ -56,6 +56,19 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, doubl
 // =============================================================================================== C ABI
 using namespace gpw;
 
+// State of gpw_eval_rho_host / gpw_eval_mat_host: device staging buffers owned by the plan, one stream per copy
+// direction and one for the kernels, so that a call's uploads, its kernels and the previous call's downloads overlap.
+struct HostIO {
+    cudaStream_t s_in = nullptr, s_out = nullptr, s_cmp = nullptr;
+    cudaEvent_t call = nullptr;                                             // the caller's stream at the start of a call
+    cudaEvent_t D_in = nullptr, rho_done = nullptr, rho_out = nullptr;      // upload of D, collocation, download of rho
+    cudaEvent_t v_in = nullptr, mat_done = nullptr, F_out = nullptr;        // upload of v, integration, download of F
+    double *D = nullptr, *F = nullptr;
+    double *rho[GPW_MAX_LEVEL] = {nullptr}, *v[GPW_MAX_LEVEL] = {nullptr};
+    int ncomp = 0;                                                          // components the level buffers hold
+    long bytes = 0;
+};
+
 struct gpw_plan {
     HostPlan *hp = nullptr;
     bool on_device = false;
@@ -80,6 +93,7 @@ struct gpw_plan {
     // serialised on the device -- every call first makes its stream wait for `busy`, recorded at the end of the
     // previous call on this plan, whatever stream that one ran on.
     cudaEvent_t busy = nullptr;
+    HostIO *hio = nullptr;      // staging buffers, streams and events of the host-buffer variants (first use)
 };
 
 namespace {
@@ -100,7 +114,18 @@ bool upload(T **dst, const T *src, size_t n, long &bytes, const char *what) {
     return true;
 }
 
+void free_hostio(HostIO *h) {
+    if (!h) return;
+    for (cudaStream_t s : {h->s_in, h->s_out, h->s_cmp}) if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); }
+    for (cudaEvent_t e : {h->call, h->D_in, h->rho_done, h->rho_out, h->v_in, h->mat_done, h->F_out}) if (e) cudaEventDestroy(e);
+    cudaFree(h->D); cudaFree(h->F);
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) { cudaFree(h->rho[a]); cudaFree(h->v[a]); }
+    delete h;
+}
+
 void free_device(gpw_plan *p) {
+    free_hostio(p->hio);
+    p->hio = nullptr;
     if (p->busy) cudaEventDestroy(p->busy);
     p->busy = nullptr;
     interp_free(p->interp);
@@ -315,7 +340,7 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
     out->nitem = hp->nitem;
     out->ncoef_total = (long)hp->ncoef_total[0];
     out->build_seconds = hp->build_seconds;
-    out->device_bytes = p->device_bytes + interp_bytes(p->interp);
+    out->device_bytes = p->device_bytes + interp_bytes(p->interp) + (p->hio ? p->hio->bytes : 0);
     return GPW_OK;
 }
 
@@ -401,7 +426,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     pp::PassArgs A;
     fill_pass(p, A, pp::PRE_DENS | (deriv == 2 ? pp::PRE_TAU : 0));
     A.D = D_dev;
-    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_rho: pre-pass launch")) return GPW_ECUDA;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, hp->max_L, st), "gpw_eval_rho: pre-pass launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
@@ -450,7 +475,7 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     pp::PassArgs A;
     fill_pass(p, A, pp::POST_MAT | (deriv == 2 ? pp::POST_TAU : 0));
     A.F = F_dev;
-    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_mat: post-pass launch")) return GPW_ECUDA;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, hp->max_L, st), "gpw_eval_mat: post-pass launch")) return GPW_ECUDA;
     if (p->timing) cudaEventRecord(p->ev[1][2], st);
     if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat: kernel launch")) return GPW_ECUDA;
     return end_call(p, st, "gpw_eval_mat");
@@ -479,8 +504,109 @@ int gpw_eval_grad(gpw_plan *p, const double *const *v_dev, int deriv, const doub
     pp::PassArgs A;
     fill_pass(p, A, pp::POST_GRAD);
     A.D = D_dev; A.grad = grad_dev;
-    if (!cuda_ok(launch_pair_pass(A, hp->max_l, st), "gpw_eval_grad: post-pass launch")) return GPW_ECUDA;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, hp->max_L, st), "gpw_eval_grad: post-pass launch")) return GPW_ECUDA;
     return end_call(p, st, "gpw_eval_grad");
+}
+
+// ---- host-buffer variants ----
+static int ensure_hostio(gpw_plan *p, int ncomp, const char *who) {
+    const HostPlan *hp = p->hp;
+    if (!p->hio) {
+        HostIO *h = new (std::nothrow) HostIO();
+        if (!h) { set_error("out of host memory"); return GPW_ENOMEM; }
+        p->hio = h;
+        bool ok = true;
+        for (cudaStream_t *s : {&h->s_in, &h->s_out, &h->s_cmp}) ok = ok && cuda_ok(cudaStreamCreateWithFlags(s, cudaStreamNonBlocking), who);
+        for (cudaEvent_t *e : {&h->call, &h->D_in, &h->rho_done, &h->rho_out, &h->v_in, &h->mat_done, &h->F_out})
+            ok = ok && cuda_ok(cudaEventCreateWithFlags(e, cudaEventDisableTiming), who);
+        const size_t nb = sizeof(double) * (size_t)hp->nao * hp->nao;
+        ok = ok && cuda_ok(cudaMalloc((void **)&h->D, nb ? nb : 8), who) && cuda_ok(cudaMalloc((void **)&h->F, nb ? nb : 8), who);
+        if (!ok) return GPW_ECUDA;
+        h->bytes += (long)(2 * nb);
+    }
+    HostIO *h = p->hio;
+    if (ncomp > h->ncomp) {   // (re)allocate the level buffers; earlier calls may still use the old ones
+        if (!cuda_ok(cudaDeviceSynchronize(), who)) return GPW_ECUDA;
+        for (int a = 0; a < hp->nlevel; a++) {
+            const size_t nb = sizeof(double) * (size_t)hp->lev[a].N[0] * hp->lev[a].N[1] * hp->lev[a].N[2];
+            cudaFree(h->rho[a]); cudaFree(h->v[a]);
+            h->rho[a] = h->v[a] = nullptr;
+            h->bytes -= (long)(2 * nb * h->ncomp);
+            if (!cuda_ok(cudaMalloc((void **)&h->rho[a], nb * ncomp), who) || !cuda_ok(cudaMalloc((void **)&h->v[a], nb * ncomp), who)) {
+                h->ncomp = 0;
+                return GPW_ENOMEM;
+            }
+            h->bytes += (long)(2 * nb * ncomp);
+        }
+        h->ncomp = ncomp;
+    }
+    return GPW_OK;
+}
+
+int gpw_eval_rho_host(gpw_plan *p, const double *D_host, int deriv, double *const *rho_host, void *cuda_stream) {
+    if (!p || !D_host || !rho_host) { set_error("gpw_eval_rho_host: null argument"); return GPW_EINVAL; }
+    if (deriv < 0 || deriv > 2) { set_error("gpw_eval_rho_host: deriv must be 0, 1 or 2"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_rho_host: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++)
+        if (!rho_host[a]) { set_error("gpw_eval_rho_host: null level pointer"); return GPW_EINVAL; }
+    const int ncomp = deriv == 0 ? 1 : (deriv == 1 ? 4 : 5);
+    if (const int rc = ensure_hostio(p, ncomp, "gpw_eval_rho_host")) return rc;
+    HostIO *h = p->hio;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const char *who = "gpw_eval_rho_host";
+    bool ok = cuda_ok(cudaEventRecord(h->call, st), who);
+    // upload of D: after the caller's earlier work, and after the previous collocation has read the staging copy
+    ok = ok && cuda_ok(cudaStreamWaitEvent(h->s_in, h->call, 0), who) && cuda_ok(cudaStreamWaitEvent(h->s_in, h->rho_done, 0), who) &&
+         cuda_ok(cudaMemcpyAsync(h->D, D_host, sizeof(double) * (size_t)hp->nao * hp->nao, cudaMemcpyHostToDevice, h->s_in), who) &&
+         cuda_ok(cudaEventRecord(h->D_in, h->s_in), who);
+    // collocation: after the upload, and after the previous download has left the staging grids
+    ok = ok && cuda_ok(cudaStreamWaitEvent(h->s_cmp, h->D_in, 0), who) && cuda_ok(cudaStreamWaitEvent(h->s_cmp, h->rho_out, 0), who);
+    if (!ok) return GPW_ECUDA;
+    if (const int rc = gpw_eval_rho(p, h->D, deriv, h->rho, h->s_cmp)) return rc;
+    ok = cuda_ok(cudaEventRecord(h->rho_done, h->s_cmp), who) && cuda_ok(cudaStreamWaitEvent(h->s_out, h->rho_done, 0), who);
+    for (int a = 0; ok && a < hp->nlevel; a++) {
+        const size_t nb = sizeof(double) * (size_t)hp->lev[a].N[0] * hp->lev[a].N[1] * hp->lev[a].N[2] * ncomp;
+        ok = cuda_ok(cudaMemcpyAsync(rho_host[a], h->rho[a], nb, cudaMemcpyDeviceToHost, h->s_out), who);
+    }
+    ok = ok && cuda_ok(cudaEventRecord(h->rho_out, h->s_out), who);
+    return ok ? GPW_OK : GPW_ECUDA;
+}
+
+int gpw_eval_mat_host(gpw_plan *p, const double *const *v_host, int deriv, double *F_host, void *cuda_stream) {
+    if (!p || !v_host || !F_host) { set_error("gpw_eval_mat_host: null argument"); return GPW_EINVAL; }
+    if (deriv < 0 || deriv > 2) { set_error("gpw_eval_mat_host: deriv must be 0, 1 or 2"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_mat_host: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++)
+        if (!v_host[a]) { set_error("gpw_eval_mat_host: null level pointer"); return GPW_EINVAL; }
+    const int ncomp = deriv == 0 ? 1 : (deriv == 1 ? 4 : 5);
+    if (const int rc = ensure_hostio(p, ncomp, "gpw_eval_mat_host")) return rc;
+    HostIO *h = p->hio;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const char *who = "gpw_eval_mat_host";
+    bool ok = cuda_ok(cudaEventRecord(h->call, st), who);
+    ok = ok && cuda_ok(cudaStreamWaitEvent(h->s_in, h->call, 0), who) && cuda_ok(cudaStreamWaitEvent(h->s_in, h->mat_done, 0), who);
+    for (int a = 0; ok && a < hp->nlevel; a++) {
+        const size_t nb = sizeof(double) * (size_t)hp->lev[a].N[0] * hp->lev[a].N[1] * hp->lev[a].N[2] * ncomp;
+        ok = cuda_ok(cudaMemcpyAsync(h->v[a], v_host[a], nb, cudaMemcpyHostToDevice, h->s_in), who);
+    }
+    ok = ok && cuda_ok(cudaEventRecord(h->v_in, h->s_in), who);
+    ok = ok && cuda_ok(cudaStreamWaitEvent(h->s_cmp, h->v_in, 0), who) && cuda_ok(cudaStreamWaitEvent(h->s_cmp, h->F_out, 0), who);
+    if (!ok) return GPW_ECUDA;
+    if (const int rc = gpw_eval_mat(p, h->v, deriv, h->F, h->s_cmp)) return rc;
+    ok = cuda_ok(cudaEventRecord(h->mat_done, h->s_cmp), who) && cuda_ok(cudaStreamWaitEvent(h->s_out, h->mat_done, 0), who) &&
+         cuda_ok(cudaMemcpyAsync(F_host, h->F, sizeof(double) * (size_t)hp->nao * hp->nao, cudaMemcpyDeviceToHost, h->s_out), who) &&
+         cuda_ok(cudaEventRecord(h->F_out, h->s_out), who);
+    return ok ? GPW_OK : GPW_ECUDA;
+}
+
+int gpw_plan_wait(gpw_plan *p, void *cuda_stream) {
+    if (!p) { set_error("gpw_plan_wait: null plan"); return GPW_EINVAL; }
+    if (!p->hio) return GPW_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return cuda_ok(cudaStreamWaitEvent(st, p->hio->rho_out, 0), "gpw_plan_wait") && cuda_ok(cudaStreamWaitEvent(st, p->hio->F_out, 0), "gpw_plan_wait")
+               ? GPW_OK : GPW_ECUDA;
 }
 
 int gpw_plan_set_timing(gpw_plan *p, int enable) {
@@ -546,6 +672,25 @@ int gpw_interp_up(gpw_plan *p, const double *const *rho_dev, int ncomp, double *
     if (const int rc = begin_call(p, st, "gpw_interp_up")) return rc;
     if (const int rc = interp_up(p->hp, &p->interp, rho_dev, ncomp, rho_fine_dev, st)) return rc;
     return end_call(p, st, "gpw_interp_up");
+}
+
+static int gspace_call(gpw_plan *p, int kind, const double *in, double *out, void *cuda_stream, const char *who) {
+    if (!p || !in || !out) { set_error(std::string(who) + ": null argument"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error(std::string(who) + ": the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    if (!aligned16(in) || !aligned16(out)) { set_error(std::string(who) + ": pointers must be 16-byte aligned"); return GPW_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, who)) return rc;
+    if (const int rc = gspace_apply(p->hp, &p->interp, kind, in, out, st)) return rc;
+    return end_call(p, st, who);
+}
+int gpw_hartree(gpw_plan *p, const double *rho_fine_dev, double *vh_fine_dev, void *cuda_stream) {
+    return gspace_call(p, 0, rho_fine_dev, vh_fine_dev, cuda_stream, "gpw_hartree");
+}
+int gpw_gspace_gradient(gpw_plan *p, const double *rho_fine_dev, double *grad_fine_dev, void *cuda_stream) {
+    return gspace_call(p, 1, rho_fine_dev, grad_fine_dev, cuda_stream, "gpw_gspace_gradient");
+}
+int gpw_gspace_divergence(gpw_plan *p, const double *w_fine_dev, double *div_fine_dev, void *cuda_stream) {
+    return gspace_call(p, 2, w_fine_dev, div_fine_dev, cuda_stream, "gpw_gspace_divergence");
 }
 
 int gpw_restrict_down(gpw_plan *p, const double *v_fine_dev, int ncomp, double *const *v_dev, void *cuda_stream) {

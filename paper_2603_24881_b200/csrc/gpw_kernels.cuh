@@ -56,13 +56,20 @@ cudaError_t launch_entry_gauss(const GridParams &P, int nbrick_all, const TaskK 
                                cudaStream_t st);
 
 // pairpass.cu: pre- and post-pass (pairpass.cuh); max_l = the largest shell angular momentum of the plan
+// and max_L the largest la + lb.  The classes la + lb <= REG_LMAX of the hot path (degree offset 0) go through the
+// register form (pairpass_reg*.cu), one translation unit per direction.
 namespace pp { struct PassArgs; }
-cudaError_t launch_pair_pass(const pp::PassArgs &A, int max_l, cudaStream_t st);
+constexpr int REG_LMAX = 4;
+cudaError_t launch_pair_pass(const pp::PassArgs &A, int max_l, int max_L, cudaStream_t st);
+cudaError_t launch_pair_reg_pre(const pp::PassArgs &A, cudaStream_t st);
+cudaError_t launch_pair_reg_post(const pp::PassArgs &A, cudaStream_t st);
 
 // interp.cu: Eq. (7)-(8) with cuFFT; the state (plans, scratch) is created on first use; return a gpw_status
 struct InterpState;
 int interp_up(const HostPlan *hp, InterpState **st, const double *const *rho, int ncomp, double *fine, cudaStream_t s);
 int interp_down(const HostPlan *hp, InterpState **st, const double *fine, int ncomp, double *const *v, cudaStream_t s);
+// kind 0: Hartree potential (in, out [N]); 1: gradient (in [N], out [3][N]); 2: divergence (in [3][N], out [N]); finest mesh
+int gspace_apply(const HostPlan *hp, InterpState **st, int kind, const double *in, double *out, cudaStream_t s);
 void interp_free(InterpState *st);
 long interp_bytes(const InterpState *st);
 

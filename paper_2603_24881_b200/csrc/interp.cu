@@ -1,5 +1,6 @@
-// Inter-level Fourier combination, Eq. (7)-(8): cuFFT plus two pointwise kernels on the
-// half spectra.  Off the optimisation target (SURVEY 8(a) row a8); HBM-bound.
+// Inter-level Fourier combination, Eq. (7)-(8), and the G-space operators of the Fock build on the
+// finest mesh (Hartree potential Eq. 5-6, gradient Eq. 10, divergence Eq. 14): cuFFT plus pointwise kernels on the
+// half spectra.  Off the optimisation target (SURVEY 8(a) row a8, 8(f) item 4); HBM-bound.
 //
 //   up:   rho~(G) = sum_alpha [F(rho_alpha)](G) for |G| < G_alpha, evaluated on the finest mesh
 //   down: v_alpha = F^-1 of [F(v_fine)](G) restricted to |G| < G_alpha          (the adjoint of up)
@@ -144,6 +145,53 @@ SpecGeom geom(const HostPlan *hp, int a, double scale) {
 
 int grid_for(size_t n) { return (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8); }
 
+// ---- G-space operators on the finest mesh (Eq. 5-6, Eq. 10, Eq. 14) ----
+// G_m = 2 pi sum_i m_i b_i.  Plane waves on a Nyquist plane (|m_i| = N_i / 2) are dropped (A26): there the
+// two aliases +-N_i/2 share one grid function but not one G.
+struct GGeom {
+    int N[3];
+    double B[9];      // B[c*3+i] = 2 pi * component c of b_i
+    double scale;     // 1 / N_grid (cuFFT's forward + inverse transforms multiply by N_grid)
+};
+enum { G_HARTREE = 0, G_GRAD = 1, G_DIV = 2 };
+
+// HARTREE: out = 4 pi / |G|^2 in (0 at G = 0);  GRAD: out = i G_c in;  DIV: out (+)= i G_c in  (accumulate if c > 0)
+template <int KIND>
+__global__ void __launch_bounds__(256) k_gspace(GGeom g, int c, const cufftDoubleComplex *__restrict__ in,
+                                                cufftDoubleComplex *__restrict__ out) {
+    const int h3 = g.N[2] / 2 + 1;
+    const long long n = (long long)g.N[0] * g.N[1] * h3;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int i3 = (int)(i % h3), i2 = (int)((i / h3) % g.N[1]), i1 = (int)(i / ((long long)h3 * g.N[1]));
+        const int m1 = i1 < g.N[0] - g.N[0] / 2 ? i1 : i1 - g.N[0];
+        const int m2 = i2 < g.N[1] - g.N[1] / 2 ? i2 : i2 - g.N[1];
+        const int m3 = i3;
+        const bool nyq = 2 * abs(m1) == g.N[0] || 2 * abs(m2) == g.N[1] || 2 * abs(m3) == g.N[2];
+        double G[3];
+#pragma unroll
+        for (int x = 0; x < 3; x++) G[x] = g.B[x * 3 + 0] * m1 + g.B[x * 3 + 1] * m2 + g.B[x * 3 + 2] * m3;
+        const cufftDoubleComplex a = in[i];
+        cufftDoubleComplex o = make_cuDoubleComplex(0.0, 0.0);
+        if (KIND == G_HARTREE) {
+            const double g2 = G[0] * G[0] + G[1] * G[1] + G[2] * G[2];
+            if (!nyq && g2 > 0.0) { const double k = 4.0 * M_PI / g2 * g.scale; o.x = k * a.x; o.y = k * a.y; }
+        } else {
+            const double Gc = c == 0 ? G[0] : (c == 1 ? G[1] : G[2]);
+            if (!nyq) { const double k = Gc * g.scale; o.x = -k * a.y; o.y = k * a.x; }   // i G_c (x + i y)
+            if (KIND == G_DIV && c > 0) { const cufftDoubleComplex p = out[i]; o.x += p.x; o.y += p.y; }
+        }
+        out[i] = o;
+    }
+}
+
+GGeom ggeom(const HostPlan *hp) {
+    GGeom g;
+    for (int i = 0; i < 3; i++) g.N[i] = hp->lev[0].N[i];
+    for (int k = 0; k < 9; k++) g.B[k] = 2.0 * M_PI * hp->binv[k];
+    g.scale = 1.0 / ((double)g.N[0] * g.N[1] * g.N[2]);
+    return g;
+}
+
 }  // namespace
 
 void interp_free(InterpState *s) {
@@ -176,6 +224,35 @@ int interp_up(const HostPlan *hp, InterpState **stp, const double *const *rho, i
             !fft_ok(cufftExecZ2D(s->inv[0], s->spec_f, fine + k * nf), "gpw_interp_up: Z2D")) return GPW_ECUDA;
     }
     return cu_ok(cudaGetLastError(), "gpw_interp_up") ? GPW_OK : GPW_ECUDA;
+}
+
+int gspace_apply(const HostPlan *hp, InterpState **stp, int kind, const double *in, double *out, cudaStream_t st) {
+    const int rc = ensure(hp, stp);
+    if (rc != GPW_OK) return rc;
+    InterpState *s = *stp;
+    const int *Nf = hp->lev[0].N;
+    const size_t nf = (size_t)Nf[0] * Nf[1] * Nf[2];
+    const GGeom g = ggeom(hp);
+    const int nblk = grid_for(half_count(Nf));
+    if (!fft_ok(cufftSetStream(s->fwd[0], st), "cufftSetStream") || !fft_ok(cufftSetStream(s->inv[0], st), "cufftSetStream")) return GPW_ECUDA;
+    if (kind == G_HARTREE) {
+        if (!fft_ok(cufftExecD2Z(s->fwd[0], const_cast<double *>(in), s->spec_f), "gpw_hartree: D2Z")) return GPW_ECUDA;
+        k_gspace<G_HARTREE><<<nblk, 256, 0, st>>>(g, 0, s->spec_f, s->spec_a);
+        if (!fft_ok(cufftExecZ2D(s->inv[0], s->spec_a, out), "gpw_hartree: Z2D")) return GPW_ECUDA;
+    } else if (kind == G_GRAD) {
+        if (!fft_ok(cufftExecD2Z(s->fwd[0], const_cast<double *>(in), s->spec_f), "gpw_gspace_gradient: D2Z")) return GPW_ECUDA;
+        for (int c = 0; c < 3; c++) {
+            k_gspace<G_GRAD><<<nblk, 256, 0, st>>>(g, c, s->spec_f, s->spec_a);
+            if (!fft_ok(cufftExecZ2D(s->inv[0], s->spec_a, out + c * nf), "gpw_gspace_gradient: Z2D")) return GPW_ECUDA;
+        }
+    } else {
+        for (int c = 0; c < 3; c++) {
+            if (!fft_ok(cufftExecD2Z(s->fwd[0], const_cast<double *>(in) + c * nf, s->spec_a), "gpw_gspace_divergence: D2Z")) return GPW_ECUDA;
+            k_gspace<G_DIV><<<nblk, 256, 0, st>>>(g, c, s->spec_a, s->spec_f);
+        }
+        if (!fft_ok(cufftExecZ2D(s->inv[0], s->spec_f, out), "gpw_gspace_divergence: Z2D")) return GPW_ECUDA;
+    }
+    return cu_ok(cudaGetLastError(), "G-space operator") ? GPW_OK : GPW_ECUDA;
 }
 
 int interp_down(const HostPlan *hp, InterpState **stp, const double *fine, int ncomp, double *const *v, cudaStream_t st) {

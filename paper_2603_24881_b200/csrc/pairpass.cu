@@ -4,6 +4,11 @@
 #include "pairpass.cuh"
 
 namespace gpw {
+
+static cudaError_t launch_pair_reg(const pp::PassArgs &A, bool post, cudaStream_t st) {
+    return post ? launch_pair_reg_post(A, st) : launch_pair_reg_pre(A, st);
+}
+
 namespace {
 
 using namespace pp;
@@ -31,8 +36,24 @@ __global__ void __launch_bounds__(PP_THREADS) k_pair_pass(const __grid_constant_
 
 }  // namespace
 
-cudaError_t launch_pair_pass(const pp::PassArgs &A, int max_l, cudaStream_t st) {
-    if (A.ntask <= 0) return cudaSuccess;
+cudaError_t launch_pair_pass(const pp::PassArgs &A0, int max_l, int max_L, cudaStream_t st) {
+    if (A0.ntask <= 0) return cudaSuccess;
+    // the hot path (degree offset 0) of the classes la + lb <= REG_LMAX in the register form, one thread per pair;
+    // the larger classes and the derivative variants in the general form, eight lanes per pair
+    pp::PassArgs A = A0;
+    A.lmin_hot = 0;
+    if (A.mode & PRE_DENS) {
+        const cudaError_t e = launch_pair_reg(A, false, st);
+        if (e != cudaSuccess) return e;
+        A.lmin_hot = REG_LMAX + 1;
+    }
+    if (A.mode & POST_MAT) {
+        const cudaError_t e = launch_pair_reg(A, true, st);
+        if (e != cudaSuccess) return e;
+        A.lmin_hot = REG_LMAX + 1;
+    }
+    if (max_L < A.lmin_hot) A.mode &= ~(PRE_DENS | POST_MAT);
+    if (A.mode == 0) return cudaSuccess;
     const int nblk = (A.ntask + PP_GROUPS - 1) / PP_GROUPS;
     if (max_l <= 2) k_pair_pass<2><<<nblk, PP_THREADS, PP_GROUPS * group_doubles<2>() * sizeof(double), st>>>(A);
     else k_pair_pass<3><<<nblk, PP_THREADS, PP_GROUPS * group_doubles<3>() * sizeof(double), st>>>(A);

@@ -49,6 +49,8 @@ enum Mode : int {
 struct PassArgs {
     const TaskP *tp;
     int ntask, nao, hdiag, mode;                      // hdiag: every level's step matrix H is diagonal (S_d diagonal)
+    int lmin_hot;                                     // PRE_DENS / POST_MAT only for pairs with la + lb >= lmin_hot (the others
+                                                      // are done by the register form, pairpass_reg.cuh)
     const double *S_all;                              // [nlevel][S_TOTAL] Cartesian -> grid-index monomial maps
     long long base[NOFF][GPW_MAX_LEVEL][8];           // workspace offset of pair t of class (level, L) = base + t * ncoef_pad(L + off)
     double dV[GPW_MAX_LEVEL];
@@ -171,7 +173,9 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
     const int nq = ncoef(lb);
     const double *S = A.S_all + (size_t)p.level * S_TOTAL;
     const double s[3] = {p.PB[0] - p.PA[0], p.PB[1] - p.PA[1], p.PB[2] - p.PA[2]};
-    const int mode = A.mode;
+    int mode = A.mode;
+    if (L < A.lmin_hot) mode &= ~(PRE_DENS | POST_MAT);
+    if (mode == 0) return;
 
     // S_d between Cartesian coefficients / moments about P (in R, degree <= n) and grid-index ones (in global memory)
     auto cart_to_grid = [&](int n, double scale, double *out) {   // out[k_u] = scale sum_col S[row k_u][col] R[col]
