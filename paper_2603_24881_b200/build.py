@@ -3,7 +3,7 @@
     python -m paper_2603_24881_b200.build [--force]
 
 The library holds the host plan builder (csrc/plan.cpp) and the CUDA kernels plus the C ABI
-(csrc/gpw_api.cu, plan_device.cu, pairpass.cu, collocate.cu, integrate.cu, interp.cu); include/gpw.h is the interface.  nvcc cross-compiles without a GPU.
+(csrc/gpw_api.cu, pairs_device.cu, plan_device.cu, pairpass.cu, collocate.cu, integrate.cu, interp.cu); include/gpw.h is the interface.  nvcc cross-compiles without a GPU.
 """
 from __future__ import annotations
 
@@ -15,10 +15,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpw.so")
-SOURCES = ["plan.cpp", "plan_device.cu", "gpw_api.cu", "pairpass.cu", "pairpass_reg_pre.cu", "pairpass_reg_post.cu", "collocate.cu", "integrate.cu", "interp.cu"]
+SOURCES = ["plan.cpp", "pairs_device.cu", "plan_device.cu", "gpw_api.cu", "pairpass.cu", "pairpass_reg_pre.cu", "pairpass_reg_post.cu", "collocate.cu", "integrate.cu", "interp.cu"]
 HEADERS = ["gpw_internal.h", "gpw_math.cuh", "gpw_kernels.cuh", "pairpass.cuh", "pairpass_reg.cuh", "pairpass_reg_kernel.cuh", "plan_device.h"]
 # plan_device.cu repeats the host builder's geometric block test: no FMA contraction, so that the two agree bit for bit
-EXTRA = {"plan_device.cu": ["-fmad=false"]}
+EXTRA = {"plan_device.cu": ["-fmad=false"], "pairs_device.cu": ["-fmad=false"]}
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O3", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -77,6 +77,7 @@ struct gpw_plan {
     // device copies
     TaskK *d_taskK = nullptr;
     TaskP *d_taskP = nullptr;
+    gpw_task *d_export = nullptr;   // the pairs as gpw_plan_export_tasks returns them (screened on the device)
     DeviceLists lists;          // visit / brick lists and work items, built on the device (plan_device.cu)
     double *d_S = nullptr;
     // per degree offset (0: Eq. 3-4; 1: nuclear gradient; 2: kinetic-energy density); offsets 1, 2 allocated on first use
@@ -133,7 +134,7 @@ void free_device(gpw_plan *p) {
     for (int w = 0; w < 2; w++)
         for (int k = 0; k < 3; k++)
             if (p->ev[w][k]) cudaEventDestroy(p->ev[w][k]);
-    cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_S);
+    cudaFree(p->d_taskK); cudaFree(p->d_taskP); cudaFree(p->d_export); cudaFree(p->d_S);
     for (int off = 0; off < NOFF; off++) { cudaFree(p->d_coef[off]); cudaFree(p->d_mom[off]); }
     cudaFree(p->d_vg); cudaFree(p->d_eg);
     free_device_lists(&p->lists);
@@ -177,7 +178,7 @@ bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 void fill_pass(const gpw_plan *p, pp::PassArgs &A, int mode) {
     std::memset(&A, 0, sizeof(A));
     const HostPlan *hp = p->hp;
-    A.tp = p->d_taskP; A.ntask = (int)hp->task.size(); A.nao = hp->nao; A.hdiag = hp->hdiag ? 1 : 0; A.mode = mode;
+    A.tp = p->d_taskP; A.ntask = (int)hp->ntask; A.nao = hp->nao; A.hdiag = hp->hdiag ? 1 : 0; A.mode = mode;
     A.S_all = p->d_S;
     for (int off = 0; off < NOFF; off++) {
         for (int a = 0; a < GPW_MAX_LEVEL; a++)
@@ -191,7 +192,7 @@ void fill_pass(const gpw_plan *p, pp::PassArgs &A, int mode) {
 // (with their static headers) and / or the moment vector.
 int need_workspace(gpw_plan *p, int off, bool coef, bool mom, cudaStream_t st, const char *who) {
     const HostPlan *hp = p->hp;
-    const size_t nt = hp->task.size();
+    const size_t nt = (size_t)hp->ntask;
     const size_t nw = (size_t)(hp->ncoef_total[off] ? hp->ncoef_total[off] : 1);
     if (coef && !p->d_coef[off]) {
         const size_t nrec = nw + 8 * nt;
@@ -228,8 +229,9 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     int ndev = 0;
     const bool have_dev = cudaGetDeviceCount(&ndev) == cudaSuccess && ndev >= 1;
     if (!have_dev) cudaGetLastError();
-    // with a device the pairs are enumerated on the host and every list is built on the device; without one the
-    // host builds the lists too (introspection only: eval calls fail with GPW_ECUDA)
+    // with a device the host only checks the arguments and computes the level geometry and the primitive radii; pairs
+    // and lists are built on the device.  Without one the host builds everything (introspection only: eval calls fail
+    // with GPW_ECUDA)
     const int rc = build_host_plan(cell, natm, xyz, nshl, shl_atom, shl_l, shl_nprim, shl_prim_off, prim_exp,
                                    prim_coef, nlevel, mesh, tau, rel_cutoff, hermi, !have_dev, &hp);
     if (rc != GPW_OK) return rc;
@@ -243,10 +245,14 @@ int gpw_build_pairs(const double *cell, int natm, const double *xyz, int nshl, c
     cudaGetDevice(&p->device);
     bool ok = true;
     long &nb = p->device_bytes;
-    ok = ok && upload(&p->d_taskK, hp->taskK.data(), hp->taskK.size(), nb, "upload pairs");
-    ok = ok && upload(&p->d_taskP, hp->taskP.data(), hp->taskP.size(), nb, "upload pairs");
-    if (ok) {
-        const int lrc = build_device_lists(hp, &p->lists);
+    {
+        DevicePairs dp;
+        const int prc = build_device_pairs(hp, &dp);
+        if (prc != GPW_OK) { delete hp; delete p; return prc; }
+        p->d_taskK = dp.taskK; p->d_taskP = dp.taskP; p->d_export = dp.exported;
+        nb += dp.bytes - (long)(sizeof(DevTask) * (size_t)dp.ntask);
+        const int lrc = build_device_lists(hp, dp.devtask, (int)dp.ntask, &p->lists);
+        cudaFree(dp.devtask);
         if (lrc != GPW_OK) {
             free_device(p);
             delete hp;
@@ -330,7 +336,7 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
     std::memset(out, 0, sizeof(*out));
     out->nao = hp->nao; out->nshl = hp->nshl; out->nlevel = hp->nlevel; out->hermi = hp->hermi;
     out->on_device = p->on_device ? 1 : 0;
-    out->ntask = (long)hp->task.size();
+    out->ntask = hp->ntask;
     for (int a = 0; a < GPW_MAX_LEVEL; a++) {
         out->ntask_level[a] = hp->ntask_level[a];
         out->nvisit_level[a] = hp->nvisit_level[a];
@@ -347,9 +353,13 @@ int gpw_plan_info(const gpw_plan *p, gpw_info *out) {
 int gpw_plan_export_tasks(const gpw_plan *p, gpw_task *buf, long cap, long *ntask) {
     if (!p || !ntask) { set_error("gpw_plan_export_tasks: null argument"); return GPW_EINVAL; }
     const HostPlan *hp = p->hp;
-    *ntask = (long)hp->task.size();
+    *ntask = hp->ntask;
     if (!buf) return GPW_OK;
     const long n = std::min(cap, *ntask);
+    if (p->on_device) {   // screened on the device: copy the records back
+        if (n > 0 && !cuda_ok(cudaMemcpy(buf, p->d_export, sizeof(gpw_task) * (size_t)n, cudaMemcpyDeviceToHost), "gpw_plan_export_tasks")) return GPW_ECUDA;
+        return GPW_OK;
+    }
     for (long i = 0; i < n; i++) {
         const HostTask &t = hp->task[i];
         gpw_task &o = buf[i];
@@ -418,7 +428,7 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
         const size_t nb = sizeof(double) * (size_t)g.N[0] * g.N[1] * g.N[2] * ncomp;
         if (!cuda_ok(cudaMemsetAsync(rho_dev[a], 0, nb, st), "gpw_eval_rho: memset")) return GPW_ECUDA;
     }
-    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
+    const int ntask = (int)hp->ntask, nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_rho");
     if (deriv == 2)
         if (const int rc = need_workspace(pm, 2, true, false, st, "gpw_eval_rho: kinetic-energy workspace")) return rc;
@@ -455,7 +465,7 @@ int gpw_eval_mat(const gpw_plan *p, const double *const *v_dev, int deriv, doubl
     if (const int rc = begin_call(p, st, "gpw_eval_mat")) return rc;
     gpw_plan *pm = const_cast<gpw_plan *>(p);
     if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat: memset")) return GPW_ECUDA;
-    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
+    const int ntask = (int)hp->ntask, nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_mat");
     if (deriv == 2)
         if (const int rc = need_workspace(pm, 2, false, true, st, "gpw_eval_mat: kinetic-energy workspace")) return rc;
@@ -493,7 +503,7 @@ int gpw_eval_grad(gpw_plan *p, const double *const *v_dev, int deriv, const doub
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (const int rc = begin_call(p, st, "gpw_eval_grad")) return rc;
     if (!cuda_ok(cudaMemsetAsync(grad_dev, 0, sizeof(double) * 3 * (size_t)hp->natm, st), "gpw_eval_grad: memset")) return GPW_ECUDA;
-    const int ntask = (int)hp->task.size(), nitem = (int)hp->nitem;
+    const int ntask = (int)hp->ntask, nitem = (int)hp->nitem;
     if (ntask == 0 || nitem == 0) return end_call(p, st, "gpw_eval_grad");
     if (const int rc = need_workspace(p, 1, false, true, st, "gpw_eval_grad: workspace")) return rc;
     if (!cuda_ok(cudaMemsetAsync(p->d_mom[1], 0, sizeof(double) * (size_t)hp->ncoef_total[1], st), "gpw_eval_grad: memset")) return GPW_ECUDA;

@@ -116,6 +116,13 @@ struct BItem {
 };
 static_assert(sizeof(BItem) == 64, "BItem must be 64 bytes");
 
+// One primitive as the device pair screen reads it (T1 radius from the host).
+struct DevPrim {
+    double A[3];     // centre
+    double exp, coef, rad;
+    int shl, l, ao, atom;
+};
+
 struct HostTask {
     int shl_a, prim_a, shl_b, prim_b;
     int T[3];
@@ -133,7 +140,10 @@ struct HostPlan {
     std::vector<int> ao_loc;
     std::vector<LevelGeom> lev;
     std::vector<std::vector<double>> S;   // per level: Cartesian -> grid-index monomial maps, degree blocks
-    std::vector<HostTask> task;           // sorted by (level, L, enumeration order)
+    std::vector<DevPrim> prims;           // every primitive with its radius (T1)
+    long ntask = 0;                       // kept pairs (= task.size() once the host holds them)
+    std::vector<HostTask> task;           // sorted by (level, L, la, enumeration order); with a device the pairs are
+                                          // screened there (pairs_device.cu) and this stays empty
     std::vector<TaskK> taskK;
     std::vector<TaskP> taskP;
     // per degree offset `off`: workspace offset of pair i (global index) of class (level, L)
@@ -176,6 +186,6 @@ void set_error(const std::string &msg);
 int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
                     const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
                     const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
-                    double tau, double rel_cutoff, int hermi, bool build_lists, HostPlan **out);
+                    double tau, double rel_cutoff, int hermi, bool on_host, HostPlan **out);
 
 }  // namespace gpw

@@ -1,5 +1,6 @@
-// Host side of gpw_build_pairs: cutoff radii, pair screening, lattice images, level assignment and
-// per-block visit lists.  Follows DESIGN.md T1..T6 (readings of PAPER.md:59, :123-138, :162-164, :200,
+// Host side of gpw_build_pairs: argument checks, level geometry and the primitive cutoff radii (T1) always; pair
+// screening, lattice images, level assignment and per-block visit lists only when there is no CUDA device (a
+// host-only plan for introspection -- with a device these run there: pairs_device.cu, plan_device.cu).  Follows DESIGN.md T1..T6 (readings of PAPER.md:59, :123-138, :162-164, :200,
 // Alg. 4-5 at :435-561).  Plain C++17 + std::thread; no code shared with oracle/.
 #include <algorithm>
 #include <atomic>
@@ -144,7 +145,7 @@ void parallel_chunks(long n, long chunk, int nthread, F &&fn) {
 int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, const int *shl_atom,
                     const int *shl_l, const int *shl_nprim, const int *shl_prim_off,
                     const double *prim_exp, const double *prim_coef, int nlevel, const int *mesh,
-                    double tau, double rel_cutoff, int hermi, bool build_lists, HostPlan **out) {
+                    double tau, double rel_cutoff, int hermi, bool on_host, HostPlan **out) {
     const auto t_start = std::chrono::steady_clock::now();
     if (!cell || !xyz || !shl_atom || !shl_l || !shl_nprim || !shl_prim_off || !prim_exp || !prim_coef ||
         !mesh || !out) { set_error("gpw_build_pairs: null pointer argument"); return GPW_EINVAL; }
@@ -248,6 +249,22 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 prad[p] = prim_radius(shl_l[s], prim_exp[p], prim_coef[p], tau);
                 prim_shl[p] = s;
             }
+        // the primitives as the device pair screen reads them (pairs_device.cu)
+        hp->prims.resize(nprim);
+        for (int p = 0; p < nprim; p++) {
+            DevPrim &d = hp->prims[p];
+            std::memset(&d, 0, sizeof(d));
+            const int s = prim_shl[p];
+            if (s < 0) continue;   // a gap in the primitive table: radius 0, never paired
+            for (int x = 0; x < 3; x++) d.A[x] = xyz[3 * shl_atom[s] + x];
+            d.exp = prim_exp[p]; d.coef = prim_coef[p]; d.rad = prad[p];
+            d.shl = s; d.l = shl_l[s]; d.ao = hp->ao_loc[s]; d.atom = shl_atom[s];
+        }
+        if (!on_host) {   // with a device, pairs and lists are built there (pairs_device.cu, plan_device.cu)
+            hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+            *out = hp;
+            return GPW_OK;
+        }
 
         // ---- T2..T5: enumerate pairs (a, b, T), parallel over shell a ----
         int nthread = (int)std::thread::hardware_concurrency();
@@ -363,6 +380,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
         });
         const long ntask = (long)hp->task.size();
+        hp->ntask = ntask;
         hp->taskK.resize(ntask); hp->taskP.resize(ntask);
         // inside a class (level, L) the workspace offset is affine in the pair index: coef_base + i * ncoef_pad(L + off)
         long long coff[NOFF] = {0};
@@ -401,12 +419,6 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
         });
         for (int off = 0; off < NOFF; off++) hp->ncoef_total[off] = coff[off];
-        if (!build_lists) {   // the block / brick lists are built on the device (plan_device.cu)
-            hp->build_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
-            *out = hp;
-            return GPW_OK;
-        }
-
         // ---- T6: blocks of every pair ----
         std::vector<long long> lev_tile0(nlevel + 1, 0);
         for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;

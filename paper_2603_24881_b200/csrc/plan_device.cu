@@ -1,7 +1,7 @@
 // Device side of gpw_build_pairs: the block set of every pair (T6, T7; Alg. 4 l.10-13
 // and Alg. 5 at :488-561 build the same kind of lists on the GPU) and from it the collocation visit lists, the
-// integration brick lists and the work items of both grid kernels.  The pairs themselves (radii, screening,
-// level) come from the host (plan.cpp).
+// integration brick lists and the work items of both grid kernels.  The pairs themselves (screening, level) come
+// from pairs_device.cu.
 //
 // This file is compiled with -fmad=false: the geometric block test then performs exactly the IEEE operations of
 // the host builder, so a block is visited on the device iff it is on the host, bit for bit.
@@ -331,11 +331,10 @@ void free_device_lists(DeviceLists *l) {
     l->bentry = nullptr; l->brick_base = nullptr; l->bitem = nullptr;
 }
 
-int build_device_lists(const HostPlan *hp, DeviceLists *out) {
+int build_device_lists(const HostPlan *hp, const DevTask *d_task, int ntask, DeviceLists *out) {
     cudaStream_t st = 0;
     const auto t_start = std::chrono::steady_clock::now();
     Scratch S;
-    const int ntask = (int)hp->task.size();
     // ---- geometry and the pairs ----
     ListGeom G;
     std::memset(&G, 0, sizeof(G));
@@ -378,19 +377,6 @@ int build_device_lists(const HostPlan *hp, DeviceLists *out) {
     }
     int rc = GPW_OK;
     auto body = [&]() -> int {
-        DevTask *d_task = nullptr;
-        {
-            std::vector<DevTask> ht((size_t)ntask);
-            for (int i = 0; i < ntask; i++) {
-                const HostTask &t = hp->task[i];
-                DevTask &d = ht[i];
-                d.P[0] = t.P[0]; d.P[1] = t.P[1]; d.P[2] = t.P[2]; d.R = t.R;
-                d.level = t.level; d.L = t.la + t.lb; d.la = t.la; d.lb = t.lb;
-            }
-            GPW_ALLOC(&d_task, (size_t)ntask, "pairs");
-            GPW_TRY(cudaMemcpyAsync(d_task, ht.data(), sizeof(DevTask) * (size_t)ntask, cudaMemcpyHostToDevice, st), "pairs");
-            GPW_TRY(cudaStreamSynchronize(st), "pairs");
-        }
         // ---- count ----
         unsigned *nvis = nullptr, *nent = nullptr;
         long long *voff = nullptr, *eoff = nullptr;
@@ -422,7 +408,7 @@ int build_device_lists(const HostPlan *hp, DeviceLists *out) {
         k_task_lists<true><<<tgrid, 128, 0, st>>>(G, d_task, ntask, nvis, nent, voff, eoff, vkey, vval, ekey, eval, d_cls, d_ovf);
         GPW_TRY(cudaGetLastError(), "fill kernel");
         GPW_TRY(cudaStreamSynchronize(st), "fill kernel");
-        S.free_now(nvis); S.free_now(nent); S.free_now(voff); S.free_now(eoff); S.free_now(d_task);
+        S.free_now(nvis); S.free_now(nent); S.free_now(voff); S.free_now(eoff);
         // ---- visits: stable sort by (block, L); pair order is kept inside ----
         GPW_ALLOC(&vkey2, (size_t)nvisit, "visit keys");
         if (!S.alloc(&vval2, (size_t)nvisit, &nb)) return fail("visit lists", cudaErrorMemoryAllocation);

@@ -42,8 +42,31 @@ struct DeviceLists {
     double seconds = 0;
 };
 
+// One kept pair in enumeration order (pairs_device.cu, between its fill and record passes).
+struct RawPair {
+    int pa, pb, T[3], level;
+    double R, ap, pref;
+    double P[3], Bt[3];
+    int sym, pad;
+};
+
+// Device arrays written by build_device_pairs (owned by the caller afterwards; free with free_device_pairs).
+struct DevicePairs {
+    TaskK *taskK = nullptr;
+    TaskP *taskP = nullptr;
+    DevTask *devtask = nullptr;      // what the list builder reads; freed by the caller after build_device_lists
+    gpw_task *exported = nullptr;    // what gpw_plan_export_tasks copies back
+    long ntask = 0;
+    long bytes = 0;
+};
+
+// Pair screening on the device (T2-T5); fills hp->ntask, coef_base, ncoef_total, ntask_level, max_L.
+int build_device_pairs(HostPlan *hp, DevicePairs *out);
+void free_device_pairs(DevicePairs *d);
+
 // returns a gpw_status; on failure the message is in gpw_last_error() and nothing is left allocated
-int build_device_lists(const HostPlan *hp, DeviceLists *out);
+// d_task: the ntask pairs on the device, sorted by (level, L)
+int build_device_lists(const HostPlan *hp, const DevTask *d_task, int ntask, DeviceLists *out);
 void free_device_lists(DeviceLists *l);
 
 }  // namespace gpw

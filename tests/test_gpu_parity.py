@@ -319,3 +319,52 @@ def test_eval_on_a_side_stream_and_two_plans_interleaved():
         for got, want in zip(rho, ref[name][0]):
             assert relmax(got.cpu().numpy(), want) <= 1e-13
         assert relmax(F.cpu().numpy(), ref[name][1]) <= 1e-13
+
+
+def test_host_buffer_entry_points_match_the_resident_path():
+    """gpw_eval_rho_host / gpw_eval_mat_host (pinned host arrays in, host arrays out, copies on the library's own
+    streams): the same results as the device-pointer calls, also when several calls are queued before the wait."""
+    import torch
+    inp = inputs.make_small("triclinic", deriv=1)
+    plan = _plan(inp)
+    D = inp.D()
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    rho_ref = gpu_rho(plan, D, 1)
+    F_ref = gpu_mat(plan, v, 1)
+    Dh = torch.as_tensor(np.ascontiguousarray(D)).pin_memory()
+    vh = [torch.as_tensor(np.ascontiguousarray(x)).pin_memory() for x in v]
+    rho_h = [torch.full(x.shape, float("nan"), dtype=torch.float64).pin_memory() for x in v]
+    Fh = torch.full((inp.nao, inp.nao), float("nan"), dtype=torch.float64).pin_memory()
+    for _ in range(3):   # queued back to back: the staging buffers are reused without a race
+        gpw.gpw_eval_rho_host(plan, Dh, 1, rho_h)
+        gpw.gpw_eval_mat_host(plan, vh, 1, Fh)
+    gpw.gpw_plan_wait(plan)
+    torch.cuda.synchronize()
+    for a, b in zip(rho_h, rho_ref):
+        assert relmax(a.numpy(), b) <= 1e-13
+    assert relmax(Fh.numpy(), F_ref) <= 1e-13
+    # pageable memory works too (no overlap), and a different deriv reallocates the staging grids
+    rho0 = [torch.empty((1,) + tuple(x.shape[1:]), dtype=torch.float64) for x in v]
+    gpw.gpw_eval_rho_host(plan, torch.as_tensor(np.ascontiguousarray(D)), 0, rho0)
+    gpw.gpw_plan_wait(plan)
+    torch.cuda.synchronize()
+    for a, b in zip(rho0, rho_ref):
+        assert relmax(a.numpy()[0], b[0]) <= 1e-13
+
+
+@pytest.mark.parametrize("kind", ["cubic", "triclinic", "wrap", "contracted"])
+@pytest.mark.parametrize("hermi", [0, 1])
+def test_device_screened_pairs_equal_oracle_task_set(kind, hermi):
+    """Pair screening on the device (pairs_device.cu; T2-T5) against the oracle's enumeration: the same set of
+    (shell a, prim a, shell b, prim b, T, level) with the same radii; hermi = 1: the canonical half (A14)."""
+    inp = inputs.make_small(kind, hermi=hermi)
+    o = oracle.Oracle.from_inputs(inp)
+    oi, oR = o.tasks()
+    gi, gR = gpw.gpw_plan_export_tasks(_plan(inp))
+    want = {tuple(int(x) for x in r): float(R) for r, R in zip(oi, oR)}
+    if hermi:
+        want = {k: R for k, R in want.items()
+                if k[1] > k[3] or (k[1] == k[3] and (k[4], k[5], k[6]) >= (0, 0, 0))}
+    got = {tuple(int(x) for x in r): float(R) for r, R in zip(gi, gR)}
+    assert set(got) == set(want)
+    assert max(abs(got[k] - want[k]) / want[k] for k in got) <= 1e-13
