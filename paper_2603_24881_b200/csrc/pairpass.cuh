@@ -101,6 +101,8 @@ PP_HD int pidx(int n, int kx, int ky, int kz) {
 PP_HD double pget(const double *p, int n, int kx, int ky, int kz) {
     return (kx < 0 || ky < 0 || kz < 0 || kx + ky + kz > n) ? 0.0 : p[pidx(n, kx, ky, kz)];
 }
+// offset of the degree block S_d: sum_{e<d} ((e+1)(e+2)/2)^2 (= s_block_off(d), in closed form)
+PP_HD int sblock(int d) { return d * (d + 1) * (d + 2) * (3 * d * d + 6 * d + 1) / 60; }
 // row / column of monomial (a,b,c) inside the degree block S_d, d = a + b + c: decreasing a, then decreasing b
 PP_HD int gidx_in_block(int a, int b, int d) {
     const int r = d - a;
@@ -114,11 +116,13 @@ PP_HD void shift_line(double *p, int n, int axis, int a, int b, double s) {
     const int m = n - a - b + 1;   // entries of the line
     double c[NMAX + 1];
     int ad[NMAX + 1];
+    // addresses along the line, by differences of pidx: x: 1;  y: (n - kz + 1) - ky;  z: tri(n + 1 - kz) - ky
+    ad[0] = axis == 0 ? pidx(n, 0, a, b) : (axis == 1 ? pidx(n, a, 0, b) : pidx(n, a, b, 0));
 #pragma unroll
-    for (int j = 0; j <= NMAX; j++) {
-        ad[j] = axis == 0 ? pidx(n, j, a, b) : (axis == 1 ? pidx(n, a, j, b) : pidx(n, a, b, j));
-        c[j] = j < m ? p[ad[j]] : 0.0;
-    }
+    for (int j = 0; j < NMAX; j++)
+        ad[j + 1] = ad[j] + (axis == 0 ? 1 : (axis == 1 ? (n - b + 1) - j : (n + 1 - j) * (n + 2 - j) / 2 - b));
+#pragma unroll
+    for (int j = 0; j <= NMAX; j++) c[j] = j < m ? p[ad[j]] : 0.0;
     if (!TRANS) {
 #pragma unroll
         for (int i = 0; i < NMAX; i++)
@@ -139,13 +143,13 @@ PP_HD void shift_line(double *p, int n, int axis, int a, int b, double s) {
 template <bool TRANS>
 PP_HD void shift_polys(double *p, int npoly, int stride, int n, const double *s, const Grp &g) {
     if (n == 0) return;
-    const int n1 = n + 1, nl = n1 * n1;
+    const int nl = n * (n + 1) / 2;   // lines with at least two entries: (a, b), a + b < n
 #pragma unroll
     for (int axis = 0; axis < 3; axis++) {
         for (int e = g.gl; e < npoly * nl; e += g.G) {
-            const int ip = e / nl, l = e - ip * nl;
-            const int a = l % n1, b = l / n1;
-            if (a + b >= n) continue;   // a + b == n: a line of one entry, nothing to do
+            const int ip = e / nl;
+            int a = e - ip * nl, b = 0;
+            while (a >= n - b) { a -= n - b; b++; }
             double *q = p + ip * stride;
             if (n <= 3) shift_line<3, TRANS>(q, n, axis, a, b, s[axis]);
             else if (n <= 6) shift_line<6, TRANS>(q, n, axis, a, b, s[axis]);
@@ -184,7 +188,7 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
             const int ky = e % n1, kz = e / n1;
             for (int kx = 0; kx <= n - ky - kz; kx++) {
                 const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
-                const double *Sd = S + s_block_off(d);
+                const double *Sd = S + sblock(d);
                 const int row = gidx_in_block(kx, ky, d);
                 double v;
                 if (A.hdiag) v = Sd[row * nd + row] * R[pidx(n, kx, ky, kz)];
@@ -204,7 +208,7 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
             const int ky = e % n1, kz = e / n1;
             for (int kx = 0; kx <= n - ky - kz; kx++) {
                 const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
-                const double *Sd = S + s_block_off(d);
+                const double *Sd = S + sblock(d);
                 const int col = gidx_in_block(kx, ky, d);
                 double v;
                 if (A.hdiag) v = Sd[col * nd + col] * m[pidx(n, kx, ky, kz)];
@@ -246,17 +250,29 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         gsync(g);   // R is reused
     };
     if (mode & PRE_DENS) {
+        // line (ky, kz) of R: component i adds its line (ky - iy, kz - iz) of q'_i, shifted by ix
         const int n = L, n1 = n + 1;
         for (int e = g.gl; e < n1 * n1; e += g.G) {
             const int ky = e % n1, kz = e / n1;
-            for (int kx = 0; kx <= n - ky - kz; kx++) {
-                double v = 0.0;
-                int i = 0;
-                for (int ix = la; ix >= 0; ix--)
-                    for (int iy = la - ix; iy >= 0; iy--, i++)
-                        v += pget(q + i * NQ, lb, kx - ix, ky - iy, kz - (la - ix - iy));
-                R[pidx(n, kx, ky, kz)] = v;
-            }
+            if (ky + kz > n) continue;
+            double acc[MAXLP + 1];
+#pragma unroll
+            for (int kx = 0; kx <= MAXLP; kx++) acc[kx] = 0.0;
+            int i = 0;
+            for (int ix = la; ix >= 0; ix--)
+                for (int iy = la - ix; iy >= 0; iy--, i++) {
+                    const int ny = ky - iy, nz = kz - (la - ix - iy);
+                    if (ny < 0 || nz < 0 || ny + nz > lb) continue;
+                    const double *ql = q + i * NQ + pidx(lb, 0, ny, nz) - ix;   // ql[kx] = q'_i[kx - ix, ny, nz]
+                    const int hi = ix + lb - ny - nz;
+#pragma unroll
+                    for (int kx = 0; kx <= MAXLP; kx++)
+                        if (kx >= ix && kx <= hi) acc[kx] += ql[kx];
+                }
+            double *Rl = R + pidx(n, 0, ky, kz);
+#pragma unroll
+            for (int kx = 0; kx <= MAXLP; kx++)
+                if (kx <= n - ky - kz) Rl[kx] = acc[kx];
         }
         finish_pre(0);
     }
@@ -298,17 +314,16 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         if (mode & POST_MAT) {
             grid_to_cart(L, scale, A.mom[0] + A.base[0][p.level][L] + (long long)t * ncoef_pad(L));
             shift_polys<true>(R, 1, 0, L, p.PA, g);
-            for (int e = g.gl; e < nca * nq; e += g.G) {   // q^_i[n] = R^[i + n]
-                const int i = e / nq, k = e - i * nq;
-                // decode k -> (nx,ny,nz) of a degree-lb polynomial by scanning (lb <= 3: at most 20 entries)
+            const int lb1 = lb + 1;
+            for (int e = g.gl; e < nca * lb1 * lb1; e += g.G) {   // q^_i[n] = R^[i + n], one line (ny, nz) of q^_i at a time
+                const int i = e / (lb1 * lb1), l = e - i * lb1 * lb1;
+                const int ny = l % lb1, nz = l / lb1;
+                if (ny + nz > lb) continue;
                 int ix, iy, iz;
                 comp_of(la, i, ix, iy, iz);
-                int nx = 0, ny = 0, nz = 0, c = 0;
-                for (int z = 0; z <= lb; z++)
-                    for (int y = 0; y <= lb - z; y++)
-                        for (int x = 0; x <= lb - z - y; x++, c++)
-                            if (c == k) { nx = x; ny = y; nz = z; }
-                q[i * NQ + k] = R[pidx(L, ix + nx, iy + ny, iz + nz)];
+                double *ql = q + i * NQ + pidx(lb, 0, ny, nz);
+                const double *Rl = R + pidx(L, ix, iy + ny, iz + nz);
+                for (int nx = 0; nx <= lb - ny - nz; nx++) ql[nx] = Rl[nx];
             }
             first = false;
             gsync(g);   // R is reused
