@@ -182,6 +182,10 @@ def main():
                     help="override the config's derivative level (2 = meta-GGA: a fifth component, tau / v_tau)")
     ap.add_argument("--tau", type=float, default=None, help="override the screening threshold of Eq. 20 (configs: 1e-10; the paper used 1e-6)")
     ap.add_argument("--rel-cutoff", type=float, default=None, help="override the level-assignment constant (configs: 20; reading A6)")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: ONE workload sharded over the ranks (gpw_plan_set_partition: an n1 slab of every level per "
+                         "rank, partial F summed by an NCCL all-reduce inside the step; strong scaling) instead of one "
+                         "independent workload per rank")
     ap.add_argument("--impl", default="gpw", choices=["gpw", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -215,8 +219,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     W = max(3, args.warmup)
 
-    # every rank its own independent workload of the same shape (weak scaling)
-    inp = workload(rank_seed(args.config, rank))
+    # every rank its own independent workload of the same shape (weak scaling); --shard: the same workload on every
+    # rank, each evaluating its slab
+    shard = args.shard and world > 1
+    inp = workload(None if shard else rank_seed(args.config, rank))
     deriv, nc = inp.deriv, inp.ncomp
     t0 = time.time()
     plan = gpw.gpw_build_pairs(*inp.abi_args())
@@ -225,6 +231,9 @@ def main():
     assert info["on_device"]
     flops_step = 2.0 * gpw.model_flops(info, deriv)       # eval_rho + eval_mat
     flops_call = gpw.model_flops(info, deriv)
+    if shard:
+        gpw.gpw_plan_set_partition(plan, rank, world)
+        flops_step /= world      # summed over the ranks again below: the job's flops are those of the one workload
 
     # resident inputs / outputs
     C = torch.as_tensor(inp.C, device="cuda")
@@ -242,6 +251,8 @@ def main():
     def step():
         gpw.gpw_eval_rho(plan, D, deriv, rho)
         gpw.gpw_eval_mat(plan, v, deriv, F)
+        if shard:
+            dist.all_reduce(F)       # the path's one exchange: the partial Fock matrices (NCCL over NVLink)
 
     def barrier():
         if dist is not None:
@@ -384,9 +395,9 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per_step)), "ms_per_step_min": float(per_step.min()),
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": inp.name, "nao": inp.nao, "meshes": [int(m[0]) for m in inp.mesh], "deriv": deriv,
+        "config": {"workload": inp.name, "sharded": bool(shard), "nao": inp.nao, "meshes": [int(m[0]) for m in inp.mesh], "deriv": deriv,
                    "tau": inp.tau, "rel_cutoff": inp.rel_cutoff, "hermi": inp.hermi,
                    "pairs": info["ntask"], "block_visits": int(sum(info["nvisit_level"])),
                    "l2": f"inputs+outputs resident {resident_bytes / 1e6:.0f} MB > 126 MB L2, no explicit flush",

@@ -179,6 +179,21 @@ int gpw_eval_mat_host(gpw_plan *plan, const double *const *v_host, int deriv, do
 int gpw_plan_wait(gpw_plan *plan, void *cuda_stream);
 
 /*
+ * Sharding over processes, one GPU each: after gpw_plan_set_partition(plan, rank, nranks)
+ * the eval calls of this plan work on the slab of grid-block rows along n1 that `rank` owns on every level -- rows
+ * [T1 rank / nranks, T1 (rank + 1) / nranks) of the T1 = N1 / 4 rows, i.e. grid indices n1 in [n1_lo, n1_hi) as
+ * gpw_plan_partition_bounds returns them (HOST pointers).  Every process builds the same plan (pairs and lists are
+ * replicated) and passes full-size arrays:
+ *   gpw_eval_rho   writes the owned slab of every level and zero-fills the rest: no exchange is needed for rho, the
+ *                  slabs of the ranks are disjoint;
+ *   gpw_eval_mat / gpw_eval_grad   read v only inside the owned slab and return this rank's PARTIAL F / gradient:
+ *                  the caller sums them over the ranks (one all-reduce, e.g. NCCL through torch.distributed).
+ * rank = 0, nranks = 1 (the default) restores the whole.
+ */
+int gpw_plan_set_partition(gpw_plan *plan, int rank, int nranks);
+int gpw_plan_partition_bounds(const gpw_plan *plan, int level, int rank, int nranks, int *n1_lo, int *n1_hi);
+
+/*
  * Nuclear gradient (Alg. 3) of the grid energy
  *     E = sum_alpha dV_alpha sum_r [ v0(r) rho_alpha(r) + w(r) . grad rho_alpha(r) ]
  * at FIXED v0, w and fixed visit set, rho_alpha being the collocated density of gpw_eval_rho:

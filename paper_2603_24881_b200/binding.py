@@ -58,7 +58,7 @@ _lib = None
 
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_eval_grad", "gpw_interp_up", "gpw_restrict_down",
            "gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence",
-           "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait",
+           "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait", "gpw_plan_set_partition", "gpw_plan_partition_bounds",
            "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
@@ -99,6 +99,10 @@ def load_library():
     L.gpw_eval_mat_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
     L.gpw_plan_wait.restype = ctypes.c_int
     L.gpw_plan_wait.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+    L.gpw_plan_set_partition.restype = ctypes.c_int
+    L.gpw_plan_set_partition.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
+    L.gpw_plan_partition_bounds.restype = ctypes.c_int
+    L.gpw_plan_partition_bounds.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ip]
     for name in ("gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence"):
         getattr(L, name).restype = ctypes.c_int
         getattr(L, name).argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
@@ -268,6 +272,18 @@ def gpw_eval_mat_host(plan: Plan, v: Sequence, deriv: int, F, stream=None):
 def gpw_plan_wait(plan: Plan, stream=None):
     """Make the stream wait for every host-buffer call issued so far on the plan."""
     _check(load_library().gpw_plan_wait(plan._h, _stream_ptr(stream)))
+
+
+def gpw_plan_set_partition(plan: Plan, rank: int, nranks: int):
+    """Shard the eval calls: this process evaluates the n1 slab `rank` of `nranks` on every level (include/gpw.h)."""
+    _check(load_library().gpw_plan_set_partition(plan._h, int(rank), int(nranks)))
+
+
+def gpw_plan_partition_bounds(plan: Plan, level: int, rank: int, nranks: int):
+    """(n1_lo, n1_hi): the grid-index range along n1 that `rank` of `nranks` owns on `level`."""
+    lo, hi = ctypes.c_int(), ctypes.c_int()
+    _check(load_library().gpw_plan_partition_bounds(plan._h, int(level), int(rank), int(nranks), ctypes.byref(lo), ctypes.byref(hi)))
+    return lo.value, hi.value
 
 
 def gpw_eval_grad(plan: Plan, v: Sequence, deriv: int, D, grad, stream=None):

@@ -145,6 +145,10 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     if (w >= nitem) return;
     const Item it = items[w];
     const LevelGeom &g = P.lev[it.level];
+    {   // sharded plans: only the blocks of this process's n1 slab
+        const int b1 = it.tile / (g.T[2] * g.T[1]);
+        if (b1 < P.part_lo[it.level] || b1 >= P.part_hi[it.level]) return;
+    }
     const int lane = threadIdx.x & 31, grp = lane >> 2, x = lane & 3;
     double *wsm = sm + (size_t)warp * warp_doubles(DMAX, ORTHO);
     uint2 *tab = reinterpret_cast<uint2 *>(wsm + NGRP * GSTRIDE);

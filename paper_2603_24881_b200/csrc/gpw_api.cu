@@ -95,6 +95,7 @@ struct gpw_plan {
     // previous call on this plan, whatever stream that one ran on.
     cudaEvent_t busy = nullptr;
     HostIO *hio = nullptr;      // staging buffers, streams and events of the host-buffer variants (first use)
+    int part_rank = 0, part_n = 1;   // gpw_plan_set_partition: this process evaluates the n1 slab `part_rank` of `part_n`
 };
 
 namespace {
@@ -140,6 +141,12 @@ void free_device(gpw_plan *p) {
     free_device_lists(&p->lists);
 }
 
+// block rows [lo, hi) along n1 of slab `rank` of `n`: equal shares of the T1 rows, the remainder spread from the front
+void partition_rows(int T1, int rank, int n, int *lo, int *hi) {
+    *lo = (int)((long long)T1 * rank / n);
+    *hi = (int)((long long)T1 * (rank + 1) / n);
+}
+
 void fill_params(const gpw_plan *p, GridParams &P, double *const *grids, int off = 0, size_t comp = 0) {
     std::memset(&P, 0, sizeof(P));
     const HostPlan *hp = p->hp;
@@ -154,6 +161,7 @@ void fill_params(const gpw_plan *p, GridParams &P, double *const *grids, int off
         // comp: the launch works on component `comp` of every level's array (the fifth component of deriv = 2)
         P.grid[a] = grids[a] ? grids[a] + comp * (size_t)hp->lev[a].N[0] * hp->lev[a].N[1] * hp->lev[a].N[2] : nullptr;
         for (int L = 0; L < 8; L++) P.coef_base[a][L] = hp->coef_base[off][a][L];
+        partition_rows(hp->lev[a].T[0], p->part_rank, p->part_n, &P.part_lo[a], &P.part_hi[a]);
     }
 }
 
@@ -617,6 +625,25 @@ int gpw_plan_wait(gpw_plan *p, void *cuda_stream) {
     cudaStream_t st = (cudaStream_t)cuda_stream;
     return cuda_ok(cudaStreamWaitEvent(st, p->hio->rho_out, 0), "gpw_plan_wait") && cuda_ok(cudaStreamWaitEvent(st, p->hio->F_out, 0), "gpw_plan_wait")
                ? GPW_OK : GPW_ECUDA;
+}
+
+int gpw_plan_set_partition(gpw_plan *p, int rank, int nranks) {
+    if (!p) { set_error("gpw_plan_set_partition: null plan"); return GPW_EINVAL; }
+    if (nranks < 1 || rank < 0 || rank >= nranks) { set_error("gpw_plan_set_partition: need 0 <= rank < nranks"); return GPW_EINVAL; }
+    p->part_rank = rank; p->part_n = nranks;
+    return GPW_OK;
+}
+
+int gpw_plan_partition_bounds(const gpw_plan *p, int level, int rank, int nranks, int *n1_lo, int *n1_hi) {
+    if (!p || !n1_lo || !n1_hi) { set_error("gpw_plan_partition_bounds: null argument"); return GPW_EINVAL; }
+    if (level < 0 || level >= p->hp->nlevel || nranks < 1 || rank < 0 || rank >= nranks) {
+        set_error("gpw_plan_partition_bounds: level or rank out of range");
+        return GPW_EINVAL;
+    }
+    int lo, hi;
+    partition_rows(p->hp->lev[level].T[0], rank, nranks, &lo, &hi);
+    *n1_lo = TILE * lo; *n1_hi = TILE * hi;
+    return GPW_OK;
 }
 
 int gpw_plan_set_timing(gpw_plan *p, int enable) {

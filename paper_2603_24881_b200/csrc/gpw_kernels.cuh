@@ -13,6 +13,7 @@ struct GridParams {
     const unsigned *seg[GPW_MAX_LEVEL];          // collocation: per block, start of each L segment
     const long long *brick_base[GPW_MAX_LEVEL];  // integration: per brick, start of its entry list
     double *grid[GPW_MAX_LEVEL];                 // rho (written) or v (read)
+    int part_lo[GPW_MAX_LEVEL], part_hi[GPW_MAX_LEVEL];   // block rows [lo, hi) along n1 this process owns (gpw_plan_set_partition)
     long long coef_base[GPW_MAX_LEVEL][8];       // workspace offset of pair i of class (level, L) = base + i * ncoef_pad(L + off),
                                                  // off = the degree offset of the launch
 };

@@ -154,6 +154,10 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3
     __shared__ __align__(16) double s_pair[NWARP * NGRP * 2 * 8];   // per group: two slots of one pair record
     const BItem *itp = items + blockIdx.x;
     const int level = itp->level, brick = itp->brick;
+    {   // sharded plans: only the bricks of this process's n1 slab (a brick is one block thick along n1)
+        const int k1p = brick / (P.lev[level].B[2] * P.lev[level].B[1]);
+        if (k1p < P.part_lo[level] || k1p >= P.part_hi[level]) return;
+    }
     const unsigned it_lo = itp->lo, it_hi = itp->hi;
     const long long ebase = itp->base;
     if (threadIdx.x < 8) s_seg[threadIdx.x] = itp->seg[threadIdx.x];

@@ -368,3 +368,40 @@ def test_device_screened_pairs_equal_oracle_task_set(kind, hermi):
     got = {tuple(int(x) for x in r): float(R) for r, R in zip(gi, gR)}
     assert set(got) == set(want)
     assert max(abs(got[k] - want[k]) / want[k] for k in got) <= 1e-13
+
+
+@pytest.mark.parametrize("nranks", [2, 3])
+def test_sharded_plan_slabs_sum_to_the_whole(nranks):
+    """gpw_plan_set_partition: every rank evaluates its n1 slab of every level.  Run here one rank after the other on
+    one GPU (no kernel waits for another): the rho slabs are disjoint and tile the grid, the partial F and gradients
+    sum to the unsharded result."""
+    inp = inputs.make_small("triclinic", deriv=1)
+    plan = _plan(inp)
+    D = inp.D()
+    v = [inp.v(l) for l in range(inp.nlevel)]
+    rho_full, F_full = gpu_rho(plan, D, 1), gpu_mat(plan, v, 1)
+    g_full = gpu_grad(plan, v, 1, D, inp.natm)
+    rho_sum = [np.zeros_like(r) for r in rho_full]
+    F_sum, g_sum = np.zeros_like(F_full), np.zeros_like(g_full)
+    for rank in range(nranks):
+        gpw.gpw_plan_set_partition(plan, rank, nranks)
+        rho = gpu_rho(plan, D, 1)
+        for lev, r in enumerate(rho):
+            lo, hi = gpw.gpw_plan_partition_bounds(plan, lev, rank, nranks)
+            assert not np.any(r[:, :lo]) and not np.any(r[:, hi:])            # nothing outside the owned slab
+            assert np.array_equal(r[:, lo:hi], rho_full[lev][:, lo:hi])      # the slab itself: same items, same order
+            rho_sum[lev] += r
+        # v outside the owned slab is never read: poison it
+        vp = []
+        for lev, x in enumerate(v):
+            lo, hi = gpw.gpw_plan_partition_bounds(plan, lev, rank, nranks)
+            y = np.full_like(x, np.nan)
+            y[:, lo:hi] = x[:, lo:hi]
+            vp.append(y)
+        F_sum += gpu_mat(plan, vp, 1)
+        g_sum += gpu_grad(plan, vp, 1, D, inp.natm)
+    gpw.gpw_plan_set_partition(plan, 0, 1)
+    for a, b in zip(rho_sum, rho_full):
+        assert np.array_equal(a, b)
+    assert relmax(F_sum, F_full) <= 1e-13 and relmax(g_sum, g_full) <= 1e-13
+    assert np.array_equal(gpu_rho(plan, D, 1)[0], rho_full[0])               # back to the whole

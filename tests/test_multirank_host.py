@@ -73,3 +73,66 @@ def test_rank_seed_convention():
     a = inputs.make_config(0, seed=bench.rank_seed(0, 1))
     b = inputs.make_config(0)
     assert a.nao == b.nao and not np.array_equal(a.prim_exp, b.prim_exp)
+
+
+def _shard_worker(rank, world, port, out):
+    """The sharded mode of the path (gpw_plan_set_partition): every rank builds the SAME plan and owns one n1 slab of
+    every level; the only exchange is the sum of the partial F.  Here, without a device, the ranks exchange their slab
+    bounds and a stand-in partial F over gloo (the all-reduce bench.py --shard issues over NCCL)."""
+    import torch
+    import torch.distributed as dist
+    import paper_2603_24881_b200 as gpw
+    from paper_2603_24881_b200 import inputs
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        inp = inputs.make_small("triclinic")
+        plan = gpw.gpw_build_pairs(*inp.abi_args())
+        gpw.gpw_plan_set_partition(plan, rank, world)
+        bounds = [gpw.gpw_plan_partition_bounds(plan, lev, rank, world) for lev in range(inp.nlevel)]
+        mine = torch.tensor(bounds, dtype=torch.int64)
+        gathered = [torch.zeros_like(mine) for _ in range(world)]
+        dist.all_gather(gathered, mine)
+        # stand-in for the partial F of this rank: the number of owned grid planes per level on the diagonal
+        F = torch.zeros(inp.nlevel, dtype=torch.float64)
+        for lev, (lo, hi) in enumerate(bounds):
+            F[lev] = hi - lo
+        dist.all_reduce(F, op=dist.ReduceOp.SUM)
+        out[rank] = ([g.tolist() for g in gathered], F.tolist(), [int(m[0]) for m in inp.mesh])
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_gloo_sharded_slabs_tile_every_level():
+    import torch.multiprocessing as mp
+    world = 2
+    with mp.Manager() as mgr:
+        out = mgr.dict()
+        mp.spawn(_shard_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+        res = dict(out)
+    assert set(res) == {0, 1}
+    gathered, Fsum, n1 = res[0]
+    assert res[1][0] == gathered and res[1][1] == Fsum
+    for lev, n in enumerate(n1):
+        lo0, hi0 = gathered[0][lev]
+        lo1, hi1 = gathered[1][lev]
+        assert lo0 == 0 and hi0 == lo1 and hi1 == n          # disjoint, contiguous, covering
+        assert lo1 % 4 == 0                                   # cut on a block boundary
+        assert Fsum[lev] == n                                 # the all-reduce saw every plane once
+
+
+def test_partition_argument_checks():
+    import paper_2603_24881_b200 as gpw
+    from paper_2603_24881_b200 import inputs
+    plan = gpw.gpw_build_pairs(*inputs.make_small("cubic").abi_args())
+    for rank, n in ((2, 2), (-1, 2), (0, 0)):
+        with pytest.raises(gpw.GpwError):
+            gpw.gpw_plan_set_partition(plan, rank, n)
+    # seven ranks on a mesh of few block rows: some slabs are empty, none overlaps
+    prev = 0
+    for r in range(7):
+        lo, hi = gpw.gpw_plan_partition_bounds(plan, 0, r, 7)
+        assert lo == prev and hi >= lo
+        prev = hi
+    assert prev == int(plan.mesh[0][0])
