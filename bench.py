@@ -247,6 +247,7 @@ def main():
     resident_bytes = 2 * grid_bytes + 2 * inp.nao * inp.nao * 8
 
     peak_meas, nsm = gpw.gpw_dfma_peak(0.5)
+    peak_dmma, peak_mixed = gpw.gpw_dmma_peak(0.3)
 
     def step():
         gpw.gpw_eval_rho(plan, D, deriv, rho)
@@ -411,7 +412,8 @@ def main():
                      "unit": "TFLOP/s", "frac": (executed_tflops / NOMINAL_FP64_TFLOPS) if executed_tflops else None,
                      "traffic": ncu.get("dram_bytes"),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
-                     "peak_measured_dfma": peak_meas,
+                     "peak_measured_dfma": peak_meas, "peak_measured_dmma_m8n8k4": peak_dmma,
+                     "peak_measured_dmma_plus_dfma": peak_mixed,
                      "fp64_pipe_pct_ncu": ncu.get("fp64_pipe_pct"), "ncu_capture": ncu.get("capture"), "csrc_sha": sha,
                      "frac_k_collocate": exec_frac("k_collocate", float(kt[1])), "frac_k_integrate": exec_frac("k_integrate", float(kt[2])),
                      "model_tflops": model_tflops,

@@ -257,6 +257,13 @@ int gpw_plan_get_timing(gpw_plan *plan, int which, float *ms_out);
  */
 int gpw_dfma_peak(double min_seconds, double *tflops_out, int *sm_count_out);
 
+/*
+ * Measurement aid: the same for the FP64 tensor-core path (mma.sync.m8n8k4.f64, eight independent accumulator tiles
+ * per warp): TFLOP/s of DMMA alone and of DMMA with DFMA chains issued in the same loop (flops counted per
+ * instruction issued).  The evidence behind "FP64 CUDA cores, not DMMA".  Host pointers.
+ */
+int gpw_dmma_peak(double min_seconds, double *tflops_dmma_out, double *tflops_mixed_out);
+
 void gpw_free_plan(gpw_plan *plan);
 const char *gpw_last_error(void);
 

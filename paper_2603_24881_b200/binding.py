@@ -59,7 +59,7 @@ _lib = None
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_eval_grad", "gpw_interp_up", "gpw_restrict_down",
            "gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence",
            "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait", "gpw_plan_set_partition", "gpw_plan_partition_bounds",
-           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak",
+           "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak", "gpw_dmma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
 
@@ -120,6 +120,8 @@ def load_library():
     L.gpw_plan_get_timing.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_float)]
     L.gpw_dfma_peak.restype = ctypes.c_int
     L.gpw_dfma_peak.argtypes = [ctypes.c_double, _dp, _ip]
+    L.gpw_dmma_peak.restype = ctypes.c_int
+    L.gpw_dmma_peak.argtypes = [ctypes.c_double, _dp, _dp]
     L.gpw_free_plan.restype = None
     L.gpw_free_plan.argtypes = [ctypes.c_void_p]
     _lib = L
@@ -354,6 +356,13 @@ def gpw_dfma_peak(min_seconds: float = 0.5):
     t, n = ctypes.c_double(), ctypes.c_int()
     _check(load_library().gpw_dfma_peak(float(min_seconds), ctypes.byref(t), ctypes.byref(n)))
     return t.value, n.value
+
+
+def gpw_dmma_peak(min_seconds: float = 0.3):
+    """(TFLOP/s of mma.sync.m8n8k4.f64 alone, TFLOP/s of DMMA + DFMA issued together) on the current device."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(load_library().gpw_dmma_peak(float(min_seconds), ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 # ---- flop model of SURVEY.md 8(d): what the direct evaluation of Alg. 1/2 must compute per visited point

@@ -51,6 +51,31 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, doubl
     if (s == 12345.678) out[0] = s;   // never true; keeps the chains alive
 }
 
+// FP64 tensor-core probe: mma.sync.m8n8k4.f64 (DMMA), eight independent accumulator tiles per warp; with_dfma adds
+// the DFMA chains of k_dfma_peak to the same loop.  Flops are counted per instruction issued (512 per warp-level DMMA).
+__global__ void __launch_bounds__(256) k_dmma_peak(double *out, int iters, double seed, int with_dfma) {
+    double c[8][2];
+#pragma unroll
+    for (int k = 0; k < 8; k++) { c[k][0] = seed + k; c[k][1] = seed - k; }
+    double f0 = seed + threadIdx.x, f1 = f0 + 1, f2 = f0 + 2, f3 = f0 + 3;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 0.999999, m = 0.999999, e = 1e-9;
+#pragma unroll 1
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int r = 0; r < 8; r++) {
+#pragma unroll
+            for (int k = 0; k < 8; k++)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[k][0]), "+d"(c[k][1]) : "d"(a), "d"(b));
+            if (with_dfma) { f0 = fma(f0, m, e); f1 = fma(f1, m, e); f2 = fma(f2, m, e); f3 = fma(f3, m, e); }
+        }
+    }
+    double s = (f0 + f1) + (f2 + f3);
+#pragma unroll
+    for (int k = 0; k < 8; k++) s += c[k][0] + c[k][1];
+    if (s == 12345.678) out[0] = s;
+}
+
 }  // namespace gpw
 
 // =============================================================================================== C ABI
@@ -696,6 +721,41 @@ int gpw_dfma_peak(double min_seconds, double *tflops_out, int *sm_count_out) {
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(d);
     *tflops_out = best;
+    return GPW_OK;
+}
+
+int gpw_dmma_peak(double min_seconds, double *tflops_dmma_out, double *tflops_mixed_out) {
+    if (!tflops_dmma_out || !tflops_mixed_out) { set_error("gpw_dmma_peak: null argument"); return GPW_EINVAL; }
+    int dev = 0, nsm = 0;
+    if (!cuda_ok(cudaGetDevice(&dev), "gpw_dmma_peak") ||
+        !cuda_ok(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "gpw_dmma_peak")) return GPW_ECUDA;
+    double *d = nullptr;
+    if (!cuda_ok(cudaMalloc((void **)&d, 8), "gpw_dmma_peak")) return GPW_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = nsm * 8, threads = 256;
+    for (int mixed = 0; mixed < 2; mixed++) {
+        int iters = 512;
+        double best = 0.0, spent = 0.0;
+        k_dmma_peak<<<blocks, threads>>>(d, 16, 1.0, mixed);   // warm-up
+        while (spent < min_seconds || best == 0.0) {
+            cudaEventRecord(e0);
+            k_dmma_peak<<<blocks, threads>>>(d, iters, 1.0, mixed);
+            cudaEventRecord(e1);
+            if (!cuda_ok(cudaEventSynchronize(e1), "gpw_dmma_peak")) { cudaFree(d); return GPW_ECUDA; }
+            float ms = 0;
+            cudaEventElapsedTime(&ms, e0, e1);
+            // per loop trip and warp: 64 DMMA of 512 flops; mixed: + 32 DFMA per thread = 32 * 2 * 32 flops per warp
+            const double per_warp = 64.0 * 512.0 + (mixed ? 32.0 * 2.0 * 32.0 : 0.0);
+            const double flops = per_warp * (double)iters * blocks * (threads / 32);
+            best = std::max(best, flops / (ms * 1e-3) / 1e12);
+            spent += ms * 1e-3;
+            if (ms < 20.0f) iters *= 2;
+        }
+        *(mixed ? tflops_mixed_out : tflops_dmma_out) = best;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
     return GPW_OK;
 }
 
