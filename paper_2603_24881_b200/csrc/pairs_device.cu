@@ -124,6 +124,11 @@ __global__ void __launch_bounds__(128) k_pair_enum(const __grid_constant__ PairG
     if (!FILL) cnt[e] = n;
 }
 
+__global__ void __launch_bounds__(256) k_widen_counts(const unsigned *__restrict__ in, long long n, long long *__restrict__ out) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) out[i] = in[i];
+}
+
 __global__ void __launch_bounds__(256) k_iota(unsigned *p, long long n) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i < n) p[i] = (unsigned)i;
@@ -232,11 +237,12 @@ static int build_device_pairs_body(HostPlan *hp, DevicePairs *out, Scr &S) {
     long long ntask = 0;
     {
         size_t tb = 0;
-        auto in = cub::TransformInputIterator<long long, cub::CastOp<long long>, const unsigned *>(cnt, cub::CastOp<long long>());
-        PTRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, in, off, npp, st), "scan");
+        k_widen_counts<<<(unsigned)((npp + 255) / 256), 256, 0, st>>>(cnt, npp, off);
+        PTRY(cudaGetLastError(), "scan");
+        PTRY(cub::DeviceScan::ExclusiveSum(nullptr, tb, off, off, npp, st), "scan");
         void *tmp = nullptr;
         PALLOC((char **)&tmp, tb, "scan scratch");
-        PTRY(cub::DeviceScan::ExclusiveSum(tmp, tb, in, off, npp, st), "scan");
+        PTRY(cub::DeviceScan::ExclusiveSum(tmp, tb, off, off, npp, st), "scan");
         long long last_off = 0;
         unsigned last_cnt = 0;
         int sharp = 0;
