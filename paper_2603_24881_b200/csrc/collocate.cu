@@ -129,7 +129,11 @@ __device__ __forceinline__ int group_reduce_scatter(double *a, int lane) {
 // LMAX: largest la + lb of the plan's pairs held by the instantiation.  LOFF: degree offset -- the polynomial of a pair
 // of class L has degree L + LOFF (0: density and gradient; 2: kinetic-energy density, Eq. 15, whose pair product is
 // again a polynomial times the same Gaussian, of degree L + 2).
-template <int DERIV, int LMAX, bool ORTHO, int LOFF>
+// LLO, ACC: a launch evaluates the visits of the classes LLO <= L <= LMAX only; ACC: it adds to what an earlier launch
+// wrote instead of overwriting.  The GGA collocation of plans with f shells runs as two launches -- classes L <= 4
+// (the instantiation LMAX = 4: no body that spills, straight-line segment loops, 55 kB of code) and L = 5, 6 (LLO = 5,
+// ACC) -- because the single kernel holding all seven bodies stalled on instruction fetch and spilled (profiles/r02.md).
+template <int DERIV, int LMAX, bool ORTHO, int LOFF, int LLO = 0, bool ACC = false>
 __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_collocate(const __grid_constant__ GridParams P,
                                                                    const Visit *__restrict__ visits,
                                                                    const Item *__restrict__ items, int nitem,
@@ -166,7 +170,9 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     int nch = 0;
     int kend[LMAX + 1];      // one past the last chunk of every L segment
 #pragma unroll
-    for (int L = 0; L <= LMAX; L++) {
+    for (int L = 0; L < LLO; L++) kend[L] = 0;
+#pragma unroll
+    for (int L = LLO; L <= LMAX; L++) {
         const unsigned lo = max(it.lo, __shfl_sync(0xffffffffu, myseg, L));
         const unsigned hi = min(it.hi, __shfl_sync(0xffffffffu, myseg, L + 1));
         if (lo < hi) {
@@ -180,6 +186,10 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         kend[L] = min(nch, MAXCH);
     }
     nch = min(nch, MAXCH);   // cannot bind: at most MAXVIS / NGRP full chunks + one ragged chunk per L segment
+    if (nch == 0) {          // no visit of this launch's classes in the item (the memset / the earlier launch stands)
+        cp_async_wait<0>();
+        return;
+    }
 
     ColCtx c;
     c.rec = rec;
@@ -243,6 +253,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         }
     };
     if constexpr (LMAX <= 4 || DERIV == 0) {
+        static_assert(LLO == 0, "the straight-line form starts at L = 0");
         run_segment(std::integral_constant<int, 0>{}, kend[0]);
         run_segment(std::integral_constant<int, 1>{}, kend[1]);
         run_segment(std::integral_constant<int, 2>{}, kend[2]);
@@ -263,11 +274,11 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
                 const unsigned long long v0 = vis[e.x + grp];
                 const double *s = c.slot + slot * SLOT;
                 switch ((int)(e.y & 0xffu)) {
-                    case 0: colloc_visit<0 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 1: colloc_visit<1 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 2: colloc_visit<2 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 3: colloc_visit<3 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
-                    case 4: colloc_visit<4 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 0: if constexpr (LLO <= 0) colloc_visit<0 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 1: if constexpr (LLO <= 1) colloc_visit<1 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 2: if constexpr (LLO <= 2) colloc_visit<2 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 3: if constexpr (LLO <= 3) colloc_visit<3 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
+                    case 4: if constexpr (LLO <= 4) colloc_visit<4 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
                     case 5: colloc_visit<5 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
                     default: colloc_visit<6 + LOFF, DMAX, DERIV, ORTHO>(c, v0, s, true, acc); break;
                 }
@@ -298,7 +309,11 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     double *out = P.grid[it.level] + ((size_t)c.n1 * g.N[1] + c.n2 + j) * g.N[2] + c.n3 + t0;
     if (it.single) {
 #pragma unroll
-        for (int k = 0; k < NCOMP; k++) *reinterpret_cast<double2 *>(out + k * ng) = make_double2(acc[k][0], acc[k][1]);
+        for (int k = 0; k < NCOMP; k++) {
+            double2 *o = reinterpret_cast<double2 *>(out + k * ng);
+            if constexpr (ACC) { const double2 old = *o; *o = make_double2(old.x + acc[k][0], old.y + acc[k][1]); }
+            else *o = make_double2(acc[k][0], acc[k][1]);
+        }
     } else {
 #pragma unroll
         for (int k = 0; k < NCOMP; k++) {
@@ -308,7 +323,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     }
 }
 
-template <int DERIV, int LMAX, bool ORTHO, int LOFF>
+template <int DERIV, int LMAX, bool ORTHO, int LOFF, int LLO = 0, bool ACC = false>
 cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
                    const double *rec, const double *vg, cudaStream_t st) {
     constexpr int smem = NWARP * warp_doubles(LMAX + LOFF, ORTHO) * (int)sizeof(double);
@@ -318,11 +333,11 @@ cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, 
     if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
     const bool known = dev >= 0 && dev < 64;
     if (!known || !configured_dev[dev]) {
-        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO, LOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_collocate<DERIV, LMAX, ORTHO, LOFF, LLO, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (known) configured_dev[dev] = true;
     }
-    k_collocate<DERIV, LMAX, ORTHO, LOFF><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
+    k_collocate<DERIV, LMAX, ORTHO, LOFF, LLO, ACC><<<(nitem + NWARP - 1) / NWARP, NWARP * 32, smem, st>>>(P, visits, items, nitem, rec, vg);
     return cudaGetLastError();
 }
 
@@ -331,7 +346,13 @@ cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items
                      const double *rec, const double *vg, int max_L, cudaStream_t st) {
     if (max_L <= 2) return launch<DERIV, 2, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
     if (max_L <= 4) return launch<DERIV, 4, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
-    return launch<DERIV, 6, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+    if constexpr (DERIV != 0) {   // two launches: classes L <= 4, then L = 5, 6 on top (see k_collocate): cfg4 28.9 -> 24.6 ms
+        const cudaError_t e = launch<DERIV, 4, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+        if (e != cudaSuccess) return e;
+        return launch<DERIV, 6, ORTHO, 0, 5, true>(P, visits, items, nitem, rec, vg, st);
+    } else {
+        return launch<DERIV, 6, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
+    }
 }
 // kinetic-energy density: value only, polynomials of degree L + 2
 template <bool ORTHO>

@@ -137,7 +137,10 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
 
 // LMAX: largest la + lb held by the instantiation.  LOFF: degree offset -- the moments of a pair of class L are
 // accumulated up to degree L + LOFF (0: Eq. 4; 1: nuclear gradient, Alg. 3; 2: kinetic-energy potential, Eq. 16).
-template <int DERIV, int LMAX, bool ORTHO, int LOFF>
+// LLO: a launch takes the entries of the classes LLO <= L <= LMAX only (the moments of all launches add up in `mom`).
+// Plans with f shells run as two launches, classes L <= 4 (the instantiation LMAX = 4: smaller code, and for deriv = 0
+// three CTAs per SM instead of two) and L = 5, 6.
+template <int DERIV, int LMAX, bool ORTHO, int LOFF, int LLO = 0>
 // deriv = 0 with f shells (L up to 6): three CTAs per SM leave 168 registers and the L = 5, 6 bodies spill; two CTAs
 // at 220 registers without spills are faster (cfg3 k_integrate 2.40 -> 2.31 ms)
 __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3) k_integrate(const __grid_constant__ GridParams P,
@@ -164,15 +167,19 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = lane >> 2;
     const BEntry *ent = entries + ebase;
     __syncthreads();   // s_seg
+    {   // nothing of this launch's classes in the item: leave before the brick is staged (uniform over the CTA)
+        const unsigned lo = max(it_lo, s_seg[LLO]), hi = min(it_hi, s_seg[LMAX + 1]);
+        if (lo >= hi) return;
+    }
 
     // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
     // warp-uniform); the chunks are dealt to the CTA's warps round robin.
-    int L = -1, cc = 0;
+    int L = LLO - 1, cc = 0;
     unsigned base = 0, hi = 0;
     auto next_chunk = [&]() -> bool {
         for (;;) {
             base += NGRP;
-            if (L < 0 || base >= hi) {
+            if (L < LLO || base >= hi) {
                 do {
                     L++;
                     if (L > LMAX) return false;
@@ -302,11 +309,11 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3
         const int deg = c0.L + LOFF;
         double *dst = mom + P.coef_base[level][c0.L] + (long long)enc.task * (((deg + 1) * (deg + 2) * (deg + 3) / 6 + 1) & ~1);
         switch (c0.L) {
-            case 0: integ_entry<0 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
-            case 1: integ_entry<1 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
-            case 2: integ_entry<2 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
-            case 3: if constexpr (LMAX >= 3) integ_entry<3 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
-            case 4: if constexpr (LMAX >= 4) integ_entry<4 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 0: if constexpr (LLO <= 0) integ_entry<0 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 1: if constexpr (LLO <= 1) integ_entry<1 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 2: if constexpr (LLO <= 2) integ_entry<2 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 3: if constexpr (LMAX >= 3 && LLO <= 3) integ_entry<3 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
+            case 4: if constexpr (LMAX >= 4 && LLO <= 4) integ_entry<4 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
             case 5: if constexpr (LMAX >= 5) integ_entry<5 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
             default: if constexpr (LMAX >= 6) integ_entry<6 + LOFF, DERIV, ORTHO>(c, enc, prs, gt, valid, dst); break;
         }
@@ -317,7 +324,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3
     cp_async_wait<0>();
 }
 
-template <int DERIV, int LMAX, bool ORTHO, int LOFF>
+template <int DERIV, int LMAX, bool ORTHO, int LOFF, int LLO = 0>
 cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                    const double *eg, double *mom, cudaStream_t st) {
     constexpr int smem = brick_doubles(DERIV ? 4 : 1, ORTHO) * (int)sizeof(double);
@@ -327,11 +334,11 @@ cudaError_t launch(const GridParams &P, const TaskK *tasks, const BEntry *entrie
     if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
     const bool known = dev >= 0 && dev < 64;
     if (!known || !configured_dev[dev]) {
-        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO, LOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        const cudaError_t e = cudaFuncSetAttribute(k_integrate<DERIV, LMAX, ORTHO, LOFF, LLO>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         if (known) configured_dev[dev] = true;
     }
-    k_integrate<DERIV, LMAX, ORTHO, LOFF><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
+    k_integrate<DERIV, LMAX, ORTHO, LOFF, LLO><<<nitem, NWARP * 32, smem, st>>>(P, tasks, entries, items, eg, mom);
     return cudaGetLastError();
 }
 
@@ -340,7 +347,10 @@ cudaError_t launch_l(const GridParams &P, const TaskK *tasks, const BEntry *entr
                      const double *eg, double *mom, int max_L, cudaStream_t st) {
     if (max_L <= 2) return launch<DERIV, 2, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
     if (max_L <= 4) return launch<DERIV, 4, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
-    return launch<DERIV, 6, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
+    // two launches (see k_integrate): measured cfg3 k_integrate 2.32 -> 2.15 ms, cfg4 25.5 -> 23.9 ms
+    const cudaError_t e = launch<DERIV, 4, ORTHO, 0>(P, tasks, entries, items, nitem, eg, mom, st);
+    if (e != cudaSuccess) return e;
+    return launch<DERIV, 6, ORTHO, 0, 5>(P, tasks, entries, items, nitem, eg, mom, st);
 }
 // moments of degree L + LOFF (nuclear gradient: LOFF = 1, value or value + gradient field; kinetic-energy
 // potential: LOFF = 2, value only)

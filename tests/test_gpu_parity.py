@@ -373,8 +373,8 @@ def test_device_screened_pairs_equal_oracle_task_set(kind, hermi):
 @pytest.mark.parametrize("nranks", [2, 3])
 def test_sharded_plan_slabs_sum_to_the_whole(nranks):
     """gpw_plan_set_partition: every rank evaluates its n1 slab of every level.  Run here one rank after the other on
-    one GPU (no kernel waits for another): the rho slabs are disjoint and tile the grid, the partial F and gradients
-    sum to the unsharded result."""
+    one GPU (no kernel waits for another): the rho slabs are disjoint, tile the grid and equal the unsharded rho to
+    rounding, the partial F and gradients sum to the unsharded result."""
     inp = inputs.make_small("triclinic", deriv=1)
     plan = _plan(inp)
     D = inp.D()
@@ -389,7 +389,8 @@ def test_sharded_plan_slabs_sum_to_the_whole(nranks):
         for lev, r in enumerate(rho):
             lo, hi = gpw.gpw_plan_partition_bounds(plan, lev, rank, nranks)
             assert not np.any(r[:, :lo]) and not np.any(r[:, hi:])            # nothing outside the owned slab
-            assert np.array_equal(r[:, lo:hi], rho_full[lev][:, lo:hi])      # the slab itself: same items, same order
+            if hi > lo:                                                       # the slab itself: the same work items
+                assert relmax(r[:, lo:hi], rho_full[lev][:, lo:hi]) <= 1e-13  # (atomics on split blocks: not bit for bit)
             rho_sum[lev] += r
         # v outside the owned slab is never read: poison it
         vp = []
@@ -402,6 +403,6 @@ def test_sharded_plan_slabs_sum_to_the_whole(nranks):
         g_sum += gpu_grad(plan, vp, 1, D, inp.natm)
     gpw.gpw_plan_set_partition(plan, 0, 1)
     for a, b in zip(rho_sum, rho_full):
-        assert np.array_equal(a, b)
+        assert relmax(a, b) <= 1e-13
     assert relmax(F_sum, F_full) <= 1e-13 and relmax(g_sum, g_full) <= 1e-13
-    assert np.array_equal(gpu_rho(plan, D, 1)[0], rho_full[0])               # back to the whole
+    assert relmax(gpu_rho(plan, D, 1)[0], rho_full[0]) <= 1e-13              # back to the whole
