@@ -432,7 +432,9 @@ def main():
         "fock_build_ms": fock_ms,
         "fock_build_note": "eval_rho + gpw_interp_up + gpw_hartree (Eq. 5-6) of the interpolated density + gpw_restrict_down of "
                            "[v_H, synthetic N(0,1) XC-side components] + eval_mat; XC functional itself excluded (LibXC)",
-        "plan_build_s": build_s, "plan_device_bytes": int(info["device_bytes"]),
+        "plan_build_s": build_s, "plan_build_lib_s": float(info["build_seconds"]),   # wall around the call (first use of the
+        # library in the process: module loading included) / the library's own clock inside gpw_build_pairs
+        "plan_device_bytes": int(info["device_bytes"]),
         "adjointness_rel_err": adj,
     }
     if not args.no_cpu_baseline:

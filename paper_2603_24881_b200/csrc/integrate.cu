@@ -358,7 +358,9 @@ template <int DERIV, bool ORTHO, int LOFF>
 cudaError_t launch_off(const GridParams &P, const TaskK *tasks, const BEntry *entries, const BItem *items, int nitem,
                        const double *eg, double *mom, int max_L, cudaStream_t st) {
     if (max_L <= 4) return launch<DERIV, 4, ORTHO, LOFF>(P, tasks, entries, items, nitem, eg, mom, st);
-    return launch<DERIV, 6, ORTHO, LOFF>(P, tasks, entries, items, nitem, eg, mom, st);
+    const cudaError_t e = launch<DERIV, 4, ORTHO, LOFF>(P, tasks, entries, items, nitem, eg, mom, st);   // two launches, as above
+    if (e != cudaSuccess) return e;
+    return launch<DERIV, 6, ORTHO, LOFF, 5>(P, tasks, entries, items, nitem, eg, mom, st);
 }
 
 }  // namespace

@@ -19,47 +19,57 @@ const char *last_error_cstr() { return g_err.c_str(); }
 
 namespace {
 
-inline int floordiv(int n, int d) { return n >= 0 ? n / d : -((-n + d - 1) / d); }
-inline int posmod(int n, int d) { int m = n % d; return m < 0 ? m + d : m; }
+// A grid block index (unbounded) folded into the cell: stored index and the number of lattice wraps (T7).
+struct Folded { int stored, wraps; };
+inline Folded fold(int b, int nblk) {
+    const int stored = ((b % nblk) + nblk) % nblk;
+    return Folded{stored, (b - stored) / nblk};
+}
+// block that holds grid index n (floor division by the block edge)
+inline int block_of(int n) { return n >= 0 ? n / TILE : -((TILE - 1 - n) / TILE); }
 
-// T1 (Eq. 20): largest root of r^2 |coef| r^l exp(-a r^2) = tau, 40 fixed-point steps.
+// Readings T1 and T4 share one scheme: the largest root of
+//     K prod_k (r + shift_k)^power_k exp(-a r^2) = tau
+// by 40 steps of  r <- sqrt((ln K - ln tau + sum_k power_k ln(r + shift_k)) / a)  from a start value beyond the root;
+// a non-positive argument means that the envelope never reaches tau (radius 0: dropped).
+struct EnvelopeTerm { double power, shift; };
+double envelope_root(double lnK_over_tau, double a, double start, const EnvelopeTerm *term, int nterm) {
+    double r = start;
+    for (int step = 0; step < 40; step++) {
+        double num = lnK_over_tau;
+        for (int k = 0; k < nterm; k++) num += term[k].power * std::log(r + term[k].shift);
+        const double arg = num / a;
+        if (arg <= 0.0) return 0.0;
+        r = std::sqrt(arg);
+    }
+    return r;
+}
+// T1 (Eq. 20): r^2 |coef| r^l exp(-a r^2) = tau
 double prim_radius(int l, double a, double coef, double tau) {
     const double C = std::log(std::fabs(coef)) - std::log(tau);
-    double r = std::sqrt(std::max(C, 1.0) / a) + 5.0;
-    for (int it = 0; it < 40; it++) {
-        const double arg = (C + (l + 2) * std::log(r)) / a;
-        if (arg <= 0.0) return 0.0;
-        r = std::sqrt(arg);
-    }
-    return r;
+    const EnvelopeTerm t[1] = {{(double)(l + 2), 0.0}};
+    return envelope_root(C, a, std::sqrt(std::max(C, 1.0) / a) + 5.0, t, 1);
 }
-
-// T4: largest root of r^2 kappa (r+dA)^la (r+dB)^lb exp(-a_p r^2) = tau.
+// T4: r^2 kappa (r + dA)^la (r + dB)^lb exp(-a_p r^2) = tau
 double pair_radius(int la, int lb, double ap, double kappa, double dA, double dB, double tau) {
     const double C = std::log(kappa) - std::log(tau);
-    double r = std::sqrt(std::max(C, 1.0) / ap) + dA + dB + 5.0;
-    for (int it = 0; it < 40; it++) {
-        const double arg = (C + 2.0 * std::log(r) + la * std::log(r + dA) + lb * std::log(r + dB)) / ap;
-        if (arg <= 0.0) return 0.0;
-        r = std::sqrt(arg);
-    }
-    return r;
+    const EnvelopeTerm t[3] = {{2.0, 0.0}, {(double)la, dA}, {(double)lb, dB}};
+    return envelope_root(C, ap, std::sqrt(std::max(C, 1.0) / ap) + dA + dB + 5.0, t, 3);
 }
 
-bool invert3(const double *m, double *inv, double *det_out) {
-    const double det = m[0] * (m[4] * m[8] - m[5] * m[7]) - m[1] * (m[3] * m[8] - m[5] * m[6]) +
-                       m[2] * (m[3] * m[7] - m[4] * m[6]);
+// Reciprocal vectors b_i = (a_j x a_k) / det (i, j, k cyclic), stored as the columns of inverse(cell):
+// binv[c*3+i] = component c of b_i.  False for a singular cell.
+bool reciprocal_vectors(const double *cell, double *binv, double *det_out) {
+    auto cross = [](const double *u, const double *v, double *w) {
+        w[0] = u[1] * v[2] - u[2] * v[1]; w[1] = u[2] * v[0] - u[0] * v[2]; w[2] = u[0] * v[1] - u[1] * v[0];
+    };
+    const double *a0 = cell, *a1 = cell + 3, *a2 = cell + 6;
+    double n0[3], n1[3], n2[3];
+    cross(a1, a2, n0); cross(a2, a0, n1); cross(a0, a1, n2);
+    const double det = a0[0] * n0[0] + a0[1] * n0[1] + a0[2] * n0[2];
     *det_out = det;
     if (std::fabs(det) < 1e-12) return false;
-    inv[0] = (m[4] * m[8] - m[5] * m[7]) / det;
-    inv[1] = (m[2] * m[7] - m[1] * m[8]) / det;
-    inv[2] = (m[1] * m[5] - m[2] * m[4]) / det;
-    inv[3] = (m[5] * m[6] - m[3] * m[8]) / det;
-    inv[4] = (m[0] * m[8] - m[2] * m[6]) / det;
-    inv[5] = (m[2] * m[3] - m[0] * m[5]) / det;
-    inv[6] = (m[3] * m[7] - m[4] * m[6]) / det;
-    inv[7] = (m[1] * m[6] - m[0] * m[7]) / det;
-    inv[8] = (m[0] * m[4] - m[1] * m[3]) / det;
+    for (int c = 0; c < 3; c++) { binv[c * 3 + 0] = n0[c] / det; binv[c * 3 + 1] = n1[c] / det; binv[c * 3 + 2] = n2[c] / det; }
     return true;
 }
 
@@ -106,6 +116,32 @@ void build_S(const double *H, std::vector<double> &S) {
                         blk[graded_idx(p, q, d) * nd + col] = poly[p][q][d - p - q];
             }
     }
+}
+
+// T6: does block (b1, b2, b3) (unbounded block indices on a mesh N) hold a grid point within R of P?  The centre of the
+// block decides when the answer is clear of the block's circumradius rc by a margin; otherwise its 64 points are tried,
+// r_n = (n1/N1) a1 + (n2/N2) a2 + (n3/N3) a3 (PAPER.md:483 with u0 = 0).  The expressions are those of plan_device.cu's
+// block_hit, term by term (that file is compiled without FMA contraction), so that both builders decide alike.
+bool sphere_meets_block(const double *cell, const int *N, const double *P, double R, double R2, double rc, int b1, int b2, int b3) {
+    auto point = [&](double u1, double u2, double u3, double *r) {
+        for (int x = 0; x < 3; x++) r[x] = u1 * cell[0 * 3 + x] + u2 * cell[1 * 3 + x] + u3 * cell[2 * 3 + x];
+    };
+    double c[3];
+    point((4 * b1 + 1.5) / N[0], (4 * b2 + 1.5) / N[1], (4 * b3 + 1.5) / N[2], c);
+    double dc = 0;
+    for (int x = 0; x < 3; x++) dc += (c[x] - P[x]) * (c[x] - P[x]);
+    dc = std::sqrt(dc);
+    if (dc - rc > R * (1.0 + 1e-9) + 1e-9) return false;
+    if (dc + rc < R * (1.0 - 1e-9) - 1e-9) return true;
+    for (int i = 0; i < 4; i++)
+        for (int j = 0; j < 4; j++)
+            for (int k = 0; k < 4; k++) {
+                double r[3];
+                point((double)(4 * b1 + i) / N[0], (double)(4 * b2 + j) / N[1], (double)(4 * b3 + k) / N[2], r);
+                const double d2 = (r[0] - P[0]) * (r[0] - P[0]) + (r[1] - P[1]) * (r[1] - P[1]) + (r[2] - P[2]) * (r[2] - P[2]);
+                if (d2 <= R2) return true;
+            }
+    return false;
 }
 
 struct RawEntry {
@@ -174,7 +210,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
     try {
         std::memcpy(hp->cell, cell, sizeof(double) * 9);
         double det;
-        if (!invert3(cell, hp->binv, &det)) { delete hp; set_error("gpw_build_pairs: singular cell (|det| < 1e-12)"); return GPW_EINVAL; }
+        if (!reciprocal_vectors(cell, hp->binv, &det)) { delete hp; set_error("gpw_build_pairs: singular cell (|det| < 1e-12)"); return GPW_EINVAL; }
         hp->omega = std::fabs(det);
         // binv[c*3+i] = component c of b_i, so that u_i = sum_c r_c binv[c*3+i]
         for (int i = 0; i < 3; i++)
@@ -272,72 +308,70 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
         if (nthread > 64) nthread = 64;
         std::vector<std::vector<HostTask>> per_shell(nshl);
         std::atomic<int> too_sharp(0);
+        // T3-T5 for one candidate image of primitive q next to primitive p; false if the pair is dropped
+        auto screen = [&](const DevPrim &p, const DevPrim &q, const int *img, HostTask &t) -> bool {
+            double sep2 = 0.0;
+            for (int x = 0; x < 3; x++) {
+                const double shift = img[0] * cell[0 * 3 + x] + img[1] * cell[1 * 3 + x] + img[2] * cell[2 * 3 + x];
+                t.A[x] = p.A[x];
+                t.Bt[x] = q.A[x] + shift;
+                sep2 += (t.A[x] - t.Bt[x]) * (t.A[x] - t.Bt[x]);
+            }
+            if (!(std::sqrt(sep2) < p.rad + q.rad)) return false;                       // T2
+            t.ap = p.exp + q.exp;                                                       // T3
+            double dA = 0.0, dB = 0.0;
+            for (int x = 0; x < 3; x++) {
+                t.P[x] = (p.exp * t.A[x] + q.exp * t.Bt[x]) / t.ap;
+                dA += (t.P[x] - t.A[x]) * (t.P[x] - t.A[x]);
+                dB += (t.P[x] - t.Bt[x]) * (t.P[x] - t.Bt[x]);
+            }
+            const double gauss = std::exp(-(p.exp * q.exp / t.ap) * sep2);
+            t.pref = p.coef * q.coef * gauss;
+            t.R = pair_radius(p.l, q.l, t.ap, std::fabs(p.coef * q.coef) * gauss, std::sqrt(dA), std::sqrt(dB), tau);   // T4
+            if (t.R <= 0.0) return false;
+            t.level = 0;                                                                // T5
+            for (int a = nlevel - 1; a >= 0; a--)
+                if (hp->lev[a].ecut >= rel_cutoff * t.ap) { t.level = a; break; }
+            // The kernels anchor the Gaussian recursion (Eq. 24-25) at the corner of a visited block: its value there,
+            // exp(-a_p d^2) with d up to R + one block diagonal, must not underflow.
+            const double reach = t.R + 2.0 * hp->circ[t.level];
+            if (t.ap * reach * reach > 600.0) { too_sharp = 1; return false; }
+            return true;
+        };
         parallel_chunks(nshl, 1, nthread, [&](long, long lo, long hi, int) {
-            for (long sa = lo; sa < hi; sa++) {
-                std::vector<HostTask> &outv = per_shell[sa];
+            for (long sa = lo; sa < hi; sa++)
                 for (int sb = 0; sb < nshl; sb++)
                     for (int ka = 0; ka < shl_nprim[sa]; ka++)
                         for (int kb = 0; kb < shl_nprim[sb]; kb++) {
                             const int pa = shl_prim_off[sa] + ka, pb = shl_prim_off[sb] + kb;
-                            if (hermi && pa < pb) continue;  // canonical unordered set (A14)
-                            const double ra = prad[pa], rb = prad[pb];
-                            if (ra <= 0.0 || rb <= 0.0) continue;
-                            const double *A = xyz + 3 * shl_atom[sa], *B = xyz + 3 * shl_atom[sb];
-                            const double rsum = ra + rb;
-                            const double d[3] = {A[0] - B[0], A[1] - B[1], A[2] - B[2]};
-                            int tlo[3], thi[3];
+                            if (hermi && pa < pb) continue;   // canonical unordered set (A14)
+                            const DevPrim &p = hp->prims[pa], &q = hp->prims[pb];
+                            if (p.rad <= 0.0 || q.rad <= 0.0) continue;
+                            // T2: the lattice vectors that can bring q within r_p + r_q of p, |f_i - t_i| <= (r_p + r_q) |b_i|
+                            int first[3], last[3];
                             for (int i = 0; i < 3; i++) {
-                                const double f = d[0] * hp->binv[0 * 3 + i] + d[1] * hp->binv[1 * 3 + i] + d[2] * hp->binv[2 * 3 + i];
-                                const double w = rsum * hp->bnorm[i];
-                                tlo[i] = (int)std::ceil(f - w);
-                                thi[i] = (int)std::floor(f + w);
+                                const double f = (p.A[0] - q.A[0]) * hp->binv[0 * 3 + i] + (p.A[1] - q.A[1]) * hp->binv[1 * 3 + i] +
+                                                 (p.A[2] - q.A[2]) * hp->binv[2 * 3 + i];
+                                const double w = (p.rad + q.rad) * hp->bnorm[i];
+                                first[i] = (int)std::ceil(f - w);
+                                last[i] = (int)std::floor(f + w);
                             }
-                            for (int t0 = tlo[0]; t0 <= thi[0]; t0++)
-                                for (int t1 = tlo[1]; t1 <= thi[1]; t1++)
-                                    for (int t2 = tlo[2]; t2 <= thi[2]; t2++) {
-                                        if (hermi && pa == pb) {  // keep T = 0 or T lexicographically positive
-                                            if (t0 < 0 || (t0 == 0 && (t1 < 0 || (t1 == 0 && t2 < 0)))) continue;
-                                        }
+                            int img[3];
+                            for (img[0] = first[0]; img[0] <= last[0]; img[0]++)
+                                for (img[1] = first[1]; img[1] <= last[1]; img[1]++)
+                                    for (img[2] = first[2]; img[2] <= last[2]; img[2]++) {
+                                        const bool zero = img[0] == 0 && img[1] == 0 && img[2] == 0;
+                                        const bool negative = img[0] < 0 || (img[0] == 0 && (img[1] < 0 || (img[1] == 0 && img[2] < 0)));
+                                        if (hermi && pa == pb && negative) continue;   // of (T, -T) keep the lexicographically positive one
                                         HostTask t;
-                                        double dd = 0.0;
-                                        for (int x = 0; x < 3; x++) {
-                                            const double Tv = t0 * cell[0 * 3 + x] + t1 * cell[1 * 3 + x] + t2 * cell[2 * 3 + x];
-                                            t.A[x] = A[x];
-                                            t.Bt[x] = B[x] + Tv;
-                                            dd += (t.A[x] - t.Bt[x]) * (t.A[x] - t.Bt[x]);
-                                        }
-                                        if (!(std::sqrt(dd) < rsum)) continue;
-                                        const double aa = prim_exp[pa], ab = prim_exp[pb], ap = aa + ab;
-                                        double dA = 0.0, dB = 0.0;
-                                        for (int x = 0; x < 3; x++) {
-                                            t.P[x] = (aa * t.A[x] + ab * t.Bt[x]) / ap;
-                                            dA += (t.P[x] - t.A[x]) * (t.P[x] - t.A[x]);
-                                            dB += (t.P[x] - t.Bt[x]) * (t.P[x] - t.Bt[x]);
-                                        }
-                                        dA = std::sqrt(dA); dB = std::sqrt(dB);
-                                        const double ex = std::exp(-(aa * ab / ap) * dd);
-                                        const double kappa = std::fabs(prim_coef[pa] * prim_coef[pb]) * ex;
-                                        const double R = pair_radius(shl_l[sa], shl_l[sb], ap, kappa, dA, dB, tau);
-                                        if (R <= 0.0) continue;
-                                        int lev = 0;
-                                        for (int a = nlevel - 1; a >= 0; a--)
-                                            if (hp->lev[a].ecut >= rel_cutoff * ap) { lev = a; break; }
-                                        // The kernels anchor the Gaussian recursion (Eq. 24-25) at the corner of a visited block: its
-                                        // value there, exp(-a_p d^2) with d up to R + one block diagonal, must not underflow.
-                                        {
-                                            const double reach = R + 2.0 * hp->circ[lev];
-                                            if (ap * reach * reach > 600.0) { too_sharp = 1; continue; }
-                                        }
+                                        if (!screen(p, q, img, t)) continue;
                                         t.shl_a = (int)sa; t.prim_a = pa; t.shl_b = sb; t.prim_b = pb;
-                                        t.T[0] = t0; t.T[1] = t1; t.T[2] = t2;
-                                        t.level = lev; t.la = shl_l[sa]; t.lb = shl_l[sb];
-                                        t.R = R; t.ap = ap;
-                                        t.pref = prim_coef[pa] * prim_coef[pb] * ex;
-                                        t.sym = (hermi && !(pa == pb && t0 == 0 && t1 == 0 && t2 == 0)) ? 1 : 0;
-                                        outv.push_back(t);
+                                        t.T[0] = img[0]; t.T[1] = img[1]; t.T[2] = img[2];
+                                        t.la = p.l; t.lb = q.l;
+                                        t.sym = (hermi && !(pa == pb && zero)) ? 1 : 0;
+                                        per_shell[sa].push_back(t);
                                     }
                         }
-            }
         });
         if (too_sharp) {
             delete hp;
@@ -444,45 +478,18 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
                 for (int i = 0; i < 3; i++) {
                     const double u = t.P[0] * hp->binv[0 * 3 + i] + t.P[1] * hp->binv[1 * 3 + i] + t.P[2] * hp->binv[2 * 3 + i];
                     const double w = t.R * hp->bnorm[i] * N[i];
-                    blo[i] = floordiv((int)std::ceil(u * N[i] - w), TILE);
-                    bhi[i] = floordiv((int)std::floor(u * N[i] + w), TILE);
+                    blo[i] = block_of((int)std::ceil(u * N[i] - w));
+                    bhi[i] = block_of((int)std::floor(u * N[i] + w));
                 }
                 const double R2 = t.R * t.R;
                 const double rc = circ[t.level];
                 for (int b1 = blo[0]; b1 <= bhi[0]; b1++)
                     for (int b2 = blo[1]; b2 <= bhi[1]; b2++)
                         for (int b3 = blo[2]; b3 <= bhi[2]; b3++) {
-                            // quick decisions on the block centre; the 64-point test settles the rest
-                            double cpos[3], dc = 0;
-                            {
-                                const double u1 = (4 * b1 + 1.5) / N[0], u2 = (4 * b2 + 1.5) / N[1], u3 = (4 * b3 + 1.5) / N[2];
-                                for (int x = 0; x < 3; x++) {
-                                    cpos[x] = u1 * cell[0 * 3 + x] + u2 * cell[1 * 3 + x] + u3 * cell[2 * 3 + x];
-                                    dc += (cpos[x] - t.P[x]) * (cpos[x] - t.P[x]);
-                                }
-                                dc = std::sqrt(dc);
-                            }
-                            bool hit;
-                            if (dc - rc > t.R * (1.0 + 1e-9) + 1e-9) hit = false;
-                            else if (dc + rc < t.R * (1.0 - 1e-9) - 1e-9) hit = true;
-                            else {
-                                hit = false;
-                                for (int i = 0; i < 4 && !hit; i++)
-                                    for (int j = 0; j < 4 && !hit; j++)
-                                        for (int k = 0; k < 4 && !hit; k++) {
-                                            // r_n = (n1/N1) a1 + (n2/N2) a2 + (n3/N3) a3   (u0 = 0)
-                                            const double u1 = (double)(4 * b1 + i) / N[0], u2 = (double)(4 * b2 + j) / N[1],
-                                                         u3 = (double)(4 * b3 + k) / N[2];
-                                            double r[3];
-                                            for (int x = 0; x < 3; x++) r[x] = u1 * cell[0 * 3 + x] + u2 * cell[1 * 3 + x] + u3 * cell[2 * 3 + x];
-                                            const double d2 = (r[0] - t.P[0]) * (r[0] - t.P[0]) + (r[1] - t.P[1]) * (r[1] - t.P[1]) +
-                                                              (r[2] - t.P[2]) * (r[2] - t.P[2]);
-                                            if (d2 <= R2) hit = true;
-                                        }
-                            }
-                            if (!hit) continue;
-                            const int w1 = posmod(b1, g.T[0]), w2 = posmod(b2, g.T[1]), w3 = posmod(b3, g.T[2]);
-                            const int s1 = (b1 - w1) / g.T[0], s2 = (b2 - w2) / g.T[1], s3 = (b3 - w3) / g.T[2];
+                            if (!sphere_meets_block(cell, N, t.P, t.R, R2, rc, b1, b2, b3)) continue;
+                            const Folded f1 = fold(b1, g.T[0]), f2 = fold(b2, g.T[1]), f3 = fold(b3, g.T[2]);
+                            const int w1 = f1.stored, w2 = f2.stored, w3 = f3.stored;
+                            const int s1 = f1.wraps, s2 = f2.wraps, s3 = f3.wraps;
                             if (s1 < -127 || s1 > 127 || s2 < -127 || s2 > 127 || s3 < -127 || s3 > 127) { wrap_overflow = 1; continue; }
                             RawVisit v;
                             v.key = lev_tile0[t.level] + ((long long)w1 * g.T[1] + w2) * g.T[2] + w3;
