@@ -219,6 +219,10 @@ void fill_pass(const gpw_plan *p, pp::PassArgs &A, int mode) {
         A.rec[off] = p->d_coef[off]; A.mom[off] = p->d_mom[off];
     }
     for (int a = 0; a < GPW_MAX_LEVEL; a++) A.dV[a] = a < hp->nlevel ? hp->lev[a].dV : 0.0;
+    for (int a = 0; a < GPW_MAX_LEVEL; a++) {
+        A.big_lo[a] = a < hp->nlevel ? (int)hp->big_lo[a] : 0;
+        A.big_n[a] = a < hp->nlevel ? (int)(hp->big_hi[a] - hp->big_lo[a]) : 0;
+    }
 }
 
 // Workspaces of the derivative variants (degree offsets 1, 2), allocated when first needed: collocation records

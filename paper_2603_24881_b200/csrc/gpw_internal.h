@@ -163,6 +163,8 @@ struct HostPlan {
     long long nvisit_total = 0;
     double circ[GPW_MAX_LEVEL] = {0};                // circumradius of a 4x4x4 block about its centre, per level
     int max_L = 0;                                   // largest la + lb present
+    long big_lo[GPW_MAX_LEVEL] = {0}, big_hi[GPW_MAX_LEVEL] = {0};   // per level, the pairs with la + lb >= 5 (contiguous: the
+                                                     // last classes of the level in the sort order)
     bool ortho = false;                              // the lattice vectors are mutually orthogonal (every Gm diagonal)
     bool hdiag = false;                              // ... and along the Cartesian axes (every H, hence every S_d, diagonal)
     int max_l = 0;                                   // largest shell angular momentum

@@ -49,6 +49,12 @@ enum Mode : int {
 struct PassArgs {
     const TaskP *tp;
     int ntask, nao, hdiag, mode;                      // hdiag: every level's step matrix H is diagonal (S_d diagonal)
+    // the pairs a launch of the group form works on: nsel pairs in up to GPW_MAX_LEVEL ranges, pair number j of the
+    // selection being sel_lo[r] + (j - sel_cum[r]) for sel_cum[r] <= j < sel_cum[r + 1]
+    int nsel;
+    int sel_cum[GPW_MAX_LEVEL + 1];
+    int sel_lo[GPW_MAX_LEVEL];
+    int big_lo[GPW_MAX_LEVEL], big_n[GPW_MAX_LEVEL];   // per level: the pairs with la + lb >= 5
     int lmin_hot;                                     // PRE_DENS / POST_MAT only for pairs with la + lb >= lmin_hot (the others
                                                       // are done by the register form, pairpass_reg.cuh)
     const double *S_all;                              // [nlevel][S_TOTAL] Cartesian -> grid-index monomial maps
@@ -61,10 +67,46 @@ struct PassArgs {
     double *grad;                                     // [natm][3]
 };
 
+// Index tables of the polynomials of degree n <= MAXDEG (kept in shared memory by the kernel: the index arithmetic
+// they replace -- tetrahedral numbers, divisions -- was 80 % of the instructions of the first version of this pass).
+//   zt[n * 9 + kz]    position of the first coefficient with exponent kz:  tet(n + 1) - tet(n + 1 - kz)
+//   lt[tet(n) + i]    line i of a polynomial of degree n: (ky | kz << 8), kz-major -- also the (a, b) with a + b <= n
+//   gt[goff(n) + k]   position (in the kz-major order) of monomial k of the degree-graded order (degree blocks, inside a
+//                     block decreasing x, then decreasing y -- the order of the maps S_d)
+//   mt[goff(n) + k]   exponents of coefficient k of the kz-major order: x | y << 4 | z << 8
+constexpr int tet_c(int m) { return m * (m + 1) * (m + 2) / 6; }
+constexpr int goff_c(int n) { int o = 0; for (int m = 0; m < n; m++) o += ncoef(m); return o; }
+constexpr int NTAB = goff_c(MAXDEG + 1);   // 495
+struct Tables {
+    unsigned char zt[(MAXDEG + 1) * 9];
+    unsigned char gt[NTAB];
+    unsigned short lt[ncoef(MAXDEG)];
+    unsigned short mt[NTAB];
+};
+inline void fill_tables(Tables &T) {
+    for (int n = 0; n <= MAXDEG; n++) {
+        for (int kz = 0; kz <= n; kz++) T.zt[n * 9 + kz] = (unsigned char)(tet_c(n + 1) - tet_c(n + 1 - kz));
+        int i = 0, k = 0;
+        for (int kz = 0; kz <= n; kz++)
+            for (int ky = 0; ky <= n - kz; ky++) {
+                T.lt[tet_c(n) + i++] = (unsigned short)(ky | kz << 8);
+                for (int kx = 0; kx <= n - kz - ky; kx++) T.mt[goff_c(n) + k++] = (unsigned short)(kx | ky << 4 | kz << 8);
+            }
+        int gk = 0;
+        for (int d = 0; d <= n; d++)
+            for (int a = d; a >= 0; a--)
+                for (int b = d - a; b >= 0; b--) {
+                    const int c = d - a - b;
+                    T.gt[goff_c(n) + gk++] = (unsigned char)(tet_c(n + 1) - tet_c(n + 1 - c) + b * (n - c + 1) - b * (b - 1) / 2 + a);
+                }
+    }
+}
+
 struct Grp {
     int gl;          // lane within the group
     int G;           // lanes in the group (PP_G on the device, 1 on the host)
     unsigned mask;   // the group's lanes
+    const Tables *tab;
 };
 
 PP_HD void gsync(const Grp &g) {
@@ -93,14 +135,18 @@ PP_HD double gsum(double v, const Grp &g) {
 }
 
 PP_HD constexpr int tet(int m) { return m * (m + 1) * (m + 2) / 6; }
+PP_HD int goff(int n) { return n * (n + 1) * (n + 2) * (n + 3) / 24; }   // sum_{m<n} ncoef(m)
 // position of x^kx y^ky z^kz in a polynomial of total degree <= n: kz-major, then ky, then kx (= cidx of gpw_math.cuh)
-PP_HD int pidx(int n, int kx, int ky, int kz) {
-    return tet(n + 1) - tet(n + 1 - kz) + ky * (n - kz + 1) - ky * (ky - 1) / 2 + kx;
+PP_HD int pidx(const Grp &g, int n, int kx, int ky, int kz) {
+    return g.tab->zt[n * 9 + kz] + ky * (n - kz + 1) - ((ky * (ky - 1)) >> 1) + kx;
 }
 // coefficient (kx,ky,kz) of a polynomial of degree <= n, zero outside its support
-PP_HD double pget(const double *p, int n, int kx, int ky, int kz) {
-    return (kx < 0 || ky < 0 || kz < 0 || kx + ky + kz > n) ? 0.0 : p[pidx(n, kx, ky, kz)];
+PP_HD double pget(const Grp &g, const double *p, int n, int kx, int ky, int kz) {
+    return (kx < 0 || ky < 0 || kz < 0 || kx + ky + kz > n) ? 0.0 : p[pidx(g, n, kx, ky, kz)];
 }
+// floor(e / d) for the small non-negative e of this file (e < 4096, d <= 32), by a reciprocal computed once per pair
+PP_HD int recip16(int d) { return 65536 / d + 1; }
+PP_HD int divr(int e, int r) { return (e * r) >> 16; }
 // offset of the degree block S_d: sum_{e<d} ((e+1)(e+2)/2)^2 (= s_block_off(d), in closed form)
 PP_HD int sblock(int d) { return d * (d + 1) * (d + 2) * (3 * d * d + 6 * d + 1) / 60; }
 // row / column of monomial (a,b,c) inside the degree block S_d, d = a + b + c: decreasing a, then decreasing b
@@ -112,12 +158,12 @@ PP_HD int gidx_in_block(int a, int b, int d) {
 // One line of a polynomial of degree <= n along `axis`, the other two exponents being (a, b) in the order
 // (y,z), (x,z), (x,y): Taylor shift c(x) -> c(x + s) in place, or its transpose (moments of x^j -> moments of (x+s)^j).
 template <int NMAX, bool TRANS>
-PP_HD void shift_line(double *p, int n, int axis, int a, int b, double s) {
+PP_HD void shift_line(const Grp &g, double *p, int n, int axis, int a, int b, double s) {
     const int m = n - a - b + 1;   // entries of the line
     double c[NMAX + 1];
     int ad[NMAX + 1];
     // addresses along the line, by differences of pidx: x: 1;  y: (n - kz + 1) - ky;  z: tri(n + 1 - kz) - ky
-    ad[0] = axis == 0 ? pidx(n, 0, a, b) : (axis == 1 ? pidx(n, a, 0, b) : pidx(n, a, b, 0));
+    ad[0] = axis == 0 ? pidx(g, n, 0, a, b) : (axis == 1 ? pidx(g, n, a, 0, b) : pidx(g, n, a, b, 0));
 #pragma unroll
     for (int j = 0; j < NMAX; j++)
         ad[j + 1] = ad[j] + (axis == 0 ? 1 : (axis == 1 ? (n - b + 1) - j : (n + 1 - j) * (n + 2 - j) / 2 - b));
@@ -146,14 +192,15 @@ PP_HD void shift_polys(double *p, int npoly, int stride, int n, const double *s,
     const int nl = n * (n + 1) / 2;   // lines with at least two entries: (a, b), a + b < n
 #pragma unroll
     for (int axis = 0; axis < 3; axis++) {
+        const int rnl = recip16(nl);
         for (int e = g.gl; e < npoly * nl; e += g.G) {
-            const int ip = e / nl;
-            int a = e - ip * nl, b = 0;
-            while (a >= n - b) { a -= n - b; b++; }
+            const int ip = divr(e, rnl);
+            const int ab = g.tab->lt[tet(n - 1) + (e - ip * nl)];   // the lines (a, b), a + b <= n - 1
+            const int a = ab & 0xff, b = ab >> 8;
             double *q = p + ip * stride;
-            if (n <= 3) shift_line<3, TRANS>(q, n, axis, a, b, s[axis]);
-            else if (n <= 6) shift_line<6, TRANS>(q, n, axis, a, b, s[axis]);
-            else shift_line<MAXDEG, TRANS>(q, n, axis, a, b, s[axis]);
+            if (n <= 3) shift_line<3, TRANS>(g, q, n, axis, a, b, s[axis]);
+            else if (n <= 6) shift_line<6, TRANS>(g, q, n, axis, a, b, s[axis]);
+            else shift_line<MAXDEG, TRANS>(g, q, n, axis, a, b, s[axis]);
         }
         gsync(g);
     }
@@ -182,59 +229,60 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
     if (mode == 0) return;
 
     // S_d between Cartesian coefficients / moments about P (in R, degree <= n) and grid-index ones (in global memory)
+    // Coefficient k of the kz-major order has exponents mt[k]; inside its degree block d it is row gidx_in_block of S_d,
+    // and column `col` of that block is coefficient gt[tet(d) + col] of the kz-major order.
+    const Tables &T = *g.tab;
     auto cart_to_grid = [&](int n, double scale, double *out) {   // out[k_u] = scale sum_col S[row k_u][col] R[col]
-        const int n1 = n + 1;
-        for (int e = g.gl; e < n1 * n1; e += g.G) {
-            const int ky = e % n1, kz = e / n1;
-            for (int kx = 0; kx <= n - ky - kz; kx++) {
-                const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
-                const double *Sd = S + sblock(d);
-                const int row = gidx_in_block(kx, ky, d);
-                double v;
-                if (A.hdiag) v = Sd[row * nd + row] * R[pidx(n, kx, ky, kz)];
-                else {
-                    v = 0.0;
-                    int col = 0;
-                    for (int a = d; a >= 0; a--)
-                        for (int b = d - a; b >= 0; b--, col++) v = fma(Sd[row * nd + col], R[pidx(n, a, b, d - a - b)], v);
-                }
-                out[pidx(n, kx, ky, kz)] = scale * v;
+        const unsigned short *mt = T.mt + goff(n);
+        const unsigned char *gt = T.gt + goff(n);
+        for (int k = g.gl; k < ncoef(n); k += g.G) {
+            const int kx = mt[k] & 15, ky = (mt[k] >> 4) & 15, kz = mt[k] >> 8;
+            const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
+            const double *Sd = S + sblock(d);
+            const int row = gidx_in_block(kx, ky, d);
+            double v;
+            if (A.hdiag) v = Sd[row * nd + row] * R[k];
+            else {
+                v = 0.0;
+                const unsigned char *gd = gt + tet(d);
+                const double *Sr = Sd + row * nd;
+                for (int col = 0; col < nd; col++) v = fma(Sr[col], R[gd[col]], v);
             }
+            out[k] = scale * v;
         }
     };
     auto grid_to_cart = [&](int n, double scale, const double *m) {   // R[col] = scale sum_row S[row][col] m[row]
-        const int n1 = n + 1;
-        for (int e = g.gl; e < n1 * n1; e += g.G) {
-            const int ky = e % n1, kz = e / n1;
-            for (int kx = 0; kx <= n - ky - kz; kx++) {
-                const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
-                const double *Sd = S + sblock(d);
-                const int col = gidx_in_block(kx, ky, d);
-                double v;
-                if (A.hdiag) v = Sd[col * nd + col] * m[pidx(n, kx, ky, kz)];
-                else {
-                    v = 0.0;
-                    int row = 0;
-                    for (int a = d; a >= 0; a--)
-                        for (int b = d - a; b >= 0; b--, row++) v = fma(Sd[row * nd + col], m[pidx(n, a, b, d - a - b)], v);
-                }
-                R[pidx(n, kx, ky, kz)] = scale * v;
+        const unsigned short *mt = T.mt + goff(n);
+        const unsigned char *gt = T.gt + goff(n);
+        for (int k = g.gl; k < ncoef(n); k += g.G) {
+            const int kx = mt[k] & 15, ky = (mt[k] >> 4) & 15, kz = mt[k] >> 8;
+            const int d = kx + ky + kz, nd = (d + 1) * (d + 2) / 2;
+            const double *Sd = S + sblock(d);
+            const int col = gidx_in_block(kx, ky, d);
+            double v;
+            if (A.hdiag) v = Sd[col * nd + col] * m[k];
+            else {
+                v = 0.0;
+                const unsigned char *gd = gt + tet(d);
+                for (int row = 0; row < nd; row++) v = fma(Sd[row * nd + col], m[gd[row]], v);
             }
+            R[k] = scale * v;
         }
         gsync(g);
     };
+    const int rncb = recip16(ncb), rnq = recip16(nq);
 
     // ---- steps 1-2 (pre-pass, gradient): q'_i(Y) from the D block ----
     if (mode & (PRE_DENS | PRE_TAU | POST_GRAD)) {
         for (int e = g.gl; e < nca * NQ; e += g.G) q[e] = 0.0;
         gsync(g);
         for (int e = g.gl; e < nca * ncb; e += g.G) {
-            const int i = e / ncb, j = e - i * ncb;
+            const int i = divr(e, rncb), j = e - i * ncb;
             int jx, jy, jz;
             comp_of(lb, j, jx, jy, jz);
             double d = A.D[(size_t)(p.ao_a + i) * A.nao + p.ao_b + j];
             if (p.sym) d += A.D[(size_t)(p.ao_b + j) * A.nao + p.ao_a + i];
-            q[i * NQ + pidx(lb, jx, jy, jz)] = d;
+            q[i * NQ + pidx(g, lb, jx, jy, jz)] = d;
         }
         gsync(g);
         shift_polys<false>(q, nca, NQ, lb, s, g);
@@ -251,10 +299,9 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
     };
     if (mode & PRE_DENS) {
         // line (ky, kz) of R: component i adds its line (ky - iy, kz - iz) of q'_i, shifted by ix
-        const int n = L, n1 = n + 1;
-        for (int e = g.gl; e < n1 * n1; e += g.G) {
-            const int ky = e % n1, kz = e / n1;
-            if (ky + kz > n) continue;
+        const int n = L;
+        for (int e = g.gl; e < (n + 1) * (n + 2) / 2; e += g.G) {
+            const int ky = T.lt[tet(n) + e] & 0xff, kz = T.lt[tet(n) + e] >> 8;
             double acc[MAXLP + 1];
 #pragma unroll
             for (int kx = 0; kx <= MAXLP; kx++) acc[kx] = 0.0;
@@ -263,13 +310,13 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
                 for (int iy = la - ix; iy >= 0; iy--, i++) {
                     const int ny = ky - iy, nz = kz - (la - ix - iy);
                     if (ny < 0 || nz < 0 || ny + nz > lb) continue;
-                    const double *ql = q + i * NQ + pidx(lb, 0, ny, nz) - ix;   // ql[kx] = q'_i[kx - ix, ny, nz]
+                    const double *ql = q + i * NQ + pidx(g, lb, 0, ny, nz) - ix;   // ql[kx] = q'_i[kx - ix, ny, nz]
                     const int hi = ix + lb - ny - nz;
 #pragma unroll
                     for (int kx = 0; kx <= MAXLP; kx++)
                         if (kx >= ix && kx <= hi) acc[kx] += ql[kx];
                 }
-            double *Rl = R + pidx(n, 0, ky, kz);
+            double *Rl = R + pidx(g, n, 0, ky, kz);
 #pragma unroll
             for (int kx = 0; kx <= MAXLP; kx++)
                 if (kx <= n - ky - kz) Rl[kx] = acc[kx];
@@ -277,11 +324,12 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         finish_pre(0);
     }
     if (mode & PRE_TAU) {
-        const int n = L + 2, n1 = n + 1;
+        const int n = L + 2;
         const double aab2 = 2.0 * p.aa * p.ab;
-        for (int e = g.gl; e < n1 * n1; e += g.G) {
-            const int ky = e % n1, kz = e / n1;
-            for (int kx = 0; kx <= n - ky - kz; kx++) {
+        const unsigned short *mtn = T.mt + goff(n);
+        for (int k = g.gl; k < ncoef(n); k += g.G) {
+            const int kx = mtn[k] & 15, ky = (mtn[k] >> 4) & 15, kz = mtn[k] >> 8;
+            {
                 double v = 0.0;
                 int i = 0;
                 for (int ix = la; ix >= 0; ix--)
@@ -289,19 +337,19 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
                         const double *qi = q + i * NQ;
                         const int ic[3] = {ix, iy, la - ix - iy};
                         const int n0[3] = {kx - ix, ky - iy, kz - ic[2]};   // n = k - i
-                        const double q0 = pget(qi, lb, n0[0], n0[1], n0[2]);
+                        const double q0 = pget(g, qi, lb, n0[0], n0[1], n0[2]);
 #pragma unroll
                         for (int c = 0; c < 3; c++) {
                             const int e0 = c == 0, e1 = c == 1, e2 = c == 2;
-                            const double qm2 = pget(qi, lb, n0[0] - 2 * e0, n0[1] - 2 * e1, n0[2] - 2 * e2);
-                            const double qm1 = pget(qi, lb, n0[0] - e0, n0[1] - e1, n0[2] - e2);
-                            const double qp1 = pget(qi, lb, n0[0] + e0, n0[1] + e1, n0[2] + e2);
-                            const double qp2 = pget(qi, lb, n0[0] + 2 * e0, n0[1] + 2 * e1, n0[2] + 2 * e2);
+                            const double qm2 = pget(g, qi, lb, n0[0] - 2 * e0, n0[1] - 2 * e1, n0[2] - 2 * e2);
+                            const double qm1 = pget(g, qi, lb, n0[0] - e0, n0[1] - e1, n0[2] - e2);
+                            const double qp1 = pget(g, qi, lb, n0[0] + e0, n0[1] + e1, n0[2] + e2);
+                            const double qp2 = pget(g, qi, lb, n0[0] + 2 * e0, n0[1] + 2 * e1, n0[2] + 2 * e2);
                             v += aab2 * (qm2 + s[c] * qm1) - (p.ab * ic[c] + p.aa * n0[c]) * q0 -
                                  p.ab * s[c] * ic[c] * qp1 + 0.5 * ic[c] * (n0[c] + 2) * qp2;
                         }
                     }
-                R[pidx(n, kx, ky, kz)] = v;
+                R[k] = v;
             }
         }
         finish_pre(2);
@@ -314,15 +362,14 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         if (mode & POST_MAT) {
             grid_to_cart(L, scale, A.mom[0] + A.base[0][p.level][L] + (long long)t * ncoef_pad(L));
             shift_polys<true>(R, 1, 0, L, p.PA, g);
-            const int lb1 = lb + 1;
-            for (int e = g.gl; e < nca * lb1 * lb1; e += g.G) {   // q^_i[n] = R^[i + n], one line (ny, nz) of q^_i at a time
-                const int i = e / (lb1 * lb1), l = e - i * lb1 * lb1;
-                const int ny = l % lb1, nz = l / lb1;
-                if (ny + nz > lb) continue;
+            const int nlq = (lb + 1) * (lb + 2) / 2, rnlq = recip16(nlq);
+            for (int e = g.gl; e < nca * nlq; e += g.G) {   // q^_i[n] = R^[i + n], one line (ny, nz) of q^_i at a time
+                const int i = divr(e, rnlq), l = e - i * nlq;
+                const int ny = T.lt[tet(lb) + l] & 0xff, nz = T.lt[tet(lb) + l] >> 8;
                 int ix, iy, iz;
                 comp_of(la, i, ix, iy, iz);
-                double *ql = q + i * NQ + pidx(lb, 0, ny, nz);
-                const double *Rl = R + pidx(L, ix, iy + ny, iz + nz);
+                double *ql = q + i * NQ + pidx(g, lb, 0, ny, nz);
+                const double *Rl = R + pidx(g, L, ix, iy + ny, iz + nz);
                 for (int nx = 0; nx <= lb - ny - nz; nx++) ql[nx] = Rl[nx];
             }
             first = false;
@@ -334,24 +381,21 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
             shift_polys<true>(R, 1, 0, n, p.PA, g);
             const double aab2 = 2.0 * p.aa * p.ab;
             for (int e = g.gl; e < nca * nq; e += g.G) {
-                const int i = e / nq, k = e - i * nq;
+                const int i = divr(e, rnq), k = e - i * nq;
                 int ic[3];
                 comp_of(la, i, ic[0], ic[1], ic[2]);
-                int nn[3] = {0, 0, 0}, cnt = 0;
-                for (int z = 0; z <= lb; z++)
-                    for (int y = 0; y <= lb - z; y++)
-                        for (int x = 0; x <= lb - z - y; x++, cnt++)
-                            if (cnt == k) { nn[0] = x; nn[1] = y; nn[2] = z; }
+                const int mk = T.mt[goff(lb) + k];
+                const int nn[3] = {mk & 15, (mk >> 4) & 15, mk >> 8};
                 const int m0[3] = {ic[0] + nn[0], ic[1] + nn[1], ic[2] + nn[2]};   // i + n
-                const double r0 = pget(R, n, m0[0], m0[1], m0[2]);
+                const double r0 = pget(g, R, n, m0[0], m0[1], m0[2]);
                 double v = 0.0;
 #pragma unroll
                 for (int c = 0; c < 3; c++) {
                     const int e0 = c == 0, e1 = c == 1, e2 = c == 2;
-                    const double rp2 = pget(R, n, m0[0] + 2 * e0, m0[1] + 2 * e1, m0[2] + 2 * e2);
-                    const double rp1 = pget(R, n, m0[0] + e0, m0[1] + e1, m0[2] + e2);
-                    const double rm1 = pget(R, n, m0[0] - e0, m0[1] - e1, m0[2] - e2);
-                    const double rm2 = pget(R, n, m0[0] - 2 * e0, m0[1] - 2 * e1, m0[2] - 2 * e2);
+                    const double rp2 = pget(g, R, n, m0[0] + 2 * e0, m0[1] + 2 * e1, m0[2] + 2 * e2);
+                    const double rp1 = pget(g, R, n, m0[0] + e0, m0[1] + e1, m0[2] + e2);
+                    const double rm1 = pget(g, R, n, m0[0] - e0, m0[1] - e1, m0[2] - e2);
+                    const double rm2 = pget(g, R, n, m0[0] - 2 * e0, m0[1] - 2 * e1, m0[2] - 2 * e2);
                     v += aab2 * (rp2 + s[c] * rp1) - (p.ab * ic[c] + p.aa * nn[c]) * r0 - p.ab * s[c] * ic[c] * rm1 +
                          0.5 * ic[c] * nn[c] * rm2;
                 }
@@ -362,10 +406,10 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         }
         shift_polys<true>(q, nca, NQ, lb, s, g);
         for (int e = g.gl; e < nca * ncb; e += g.G) {
-            const int i = e / ncb, j = e - i * ncb;
+            const int i = divr(e, rncb), j = e - i * ncb;
             int jx, jy, jz;
             comp_of(lb, j, jx, jy, jz);
-            const double x = q[i * NQ + pidx(lb, jx, jy, jz)];
+            const double x = q[i * NQ + pidx(g, lb, jx, jy, jz)];
             add_to(A.F + (size_t)(p.ao_a + i) * A.nao + p.ao_b + j, x);
             if (p.sym) add_to(A.F + (size_t)(p.ao_b + j) * A.nao + p.ao_a + i, x);
         }
@@ -376,22 +420,19 @@ PP_HD void pair_pass(const PassArgs &A, int t, double *q, double *R, const Grp &
         shift_polys<true>(R, 1, 0, n, p.PA, g);
         double gA[3] = {0.0, 0.0, 0.0}, gB[3] = {0.0, 0.0, 0.0};
         for (int e = g.gl; e < nca * nq; e += g.G) {
-            const int i = e / nq, k = e - i * nq;
+            const int i = divr(e, rnq), k = e - i * nq;
             int ic[3];
             comp_of(la, i, ic[0], ic[1], ic[2]);
-            int nn[3] = {0, 0, 0}, cnt = 0;
-            for (int z = 0; z <= lb; z++)
-                for (int y = 0; y <= lb - z; y++)
-                    for (int x = 0; x <= lb - z - y; x++, cnt++)
-                        if (cnt == k) { nn[0] = x; nn[1] = y; nn[2] = z; }
+            const int mk = T.mt[goff(lb) + k];
+            const int nn[3] = {mk & 15, (mk >> 4) & 15, mk >> 8};
             const double qv = q[i * NQ + k];
             const int m0[3] = {ic[0] + nn[0], ic[1] + nn[1], ic[2] + nn[2]};
-            const double r0 = pget(R, n, m0[0], m0[1], m0[2]);
+            const double r0 = pget(g, R, n, m0[0], m0[1], m0[2]);
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 const int e0 = c == 0, e1 = c == 1, e2 = c == 2;
-                const double rp1 = pget(R, n, m0[0] + e0, m0[1] + e1, m0[2] + e2);
-                const double rm1 = pget(R, n, m0[0] - e0, m0[1] - e1, m0[2] - e2);
+                const double rp1 = pget(g, R, n, m0[0] + e0, m0[1] + e1, m0[2] + e2);
+                const double rm1 = pget(g, R, n, m0[0] - e0, m0[1] - e1, m0[2] - e2);
                 gA[c] -= qv * (ic[c] * rm1 - 2.0 * p.aa * rp1);
                 gB[c] -= qv * (nn[c] * rm1 - 2.0 * p.ab * (rp1 + s[c] * r0));
             }

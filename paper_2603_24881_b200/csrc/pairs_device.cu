@@ -307,6 +307,7 @@ static int build_device_pairs_body(HostPlan *hp, DevicePairs *out, Scr &S) {
         hp->max_L = std::max(hp->max_L, L);
     }
     for (int o = 0; o < NOFF; o++) hp->ncoef_total[o] = coff[o];
+    for (int a = 0; a < hp->nlevel; a++) { hp->big_lo[a] = cls_first[(a * 8 + 5) * 4]; hp->big_hi[a] = cls_first[(a * 8 + 7) * 4]; }
     PALLOC(&out->taskK, (size_t)ntask, "pair records"); PALLOC(&out->taskP, (size_t)ntask, "pair records");
     PALLOC(&out->devtask, (size_t)ntask, "pair records"); PALLOC(&out->exported, (size_t)ntask, "pair records");
     k_pair_records<<<(unsigned)((ntask + 127) / 128), 128, 0, st>>>(G, base, d_prim, raw, perm, (int)ntask, d_gm, out->taskK, out->taskP,

@@ -453,6 +453,7 @@ int build_host_plan(const double *cell, int natm, const double *xyz, int nshl, c
             }
         });
         for (int off = 0; off < NOFF; off++) hp->ncoef_total[off] = coff[off];
+        for (int a = 0; a < nlevel; a++) { hp->big_lo[a] = cls_first[(a * 8 + 5) * 4]; hp->big_hi[a] = cls_first[(a * 8 + 7) * 4]; }
         // ---- T6: blocks of every pair ----
         std::vector<long long> lev_tile0(nlevel + 1, 0);
         for (int a = 0; a < nlevel; a++) lev_tile0[a + 1] = lev_tile0[a] + hp->lev[a].ntile;
