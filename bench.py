@@ -392,7 +392,15 @@ def main():
         e = (ncu_all.get(f"{inp.name}:{kernel}") or {}).get("executed_fp64_flops")
         return (e / (ms * 1e-3) / 1e12 / NOMINAL_FP64_TFLOPS) if e else None
 
-    nlaunch = 4 + (2 if deriv == 2 else 0)
+    # kernels of this repository launched per step (counted from the launch logic of gpw_eval_rho / gpw_eval_mat): the
+    # register-form pre/post-pass, the group form when the plan has classes la + lb >= 5 or for deriv = 2, one collocation
+    # and one integration launch per class range (two ranges on plans with f shells; collocation splits only for deriv >= 1)
+    cls = info["nvisit_class"]
+    big = any(int(cls[:, la, lb].sum()) > 0 for la in range(4) for lb in range(4) if la + lb >= 5)
+    n_pre = 1 + (1 if (big or deriv == 2) else 0)
+    n_col = (2 if (big and deriv >= 1) else 1) + (1 if deriv == 2 else 0)
+    n_int = (2 if big else 1) * (2 if deriv == 2 else 1)
+    nlaunch = n_pre + n_col + n_int + n_pre
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
         "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per_step)), "ms_per_step_min": float(per_step.min()),
