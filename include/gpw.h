@@ -162,6 +162,24 @@ int gpw_eval_mat(const gpw_plan *plan, const double *const *v_dev, int deriv, do
                  void *cuda_stream);
 
 /*
+ * Integration without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops,
+ * harnesses that forbid it): gpw_eval_mat with the same arguments and the same result, whose scratch -- the moment
+ * workspace the integration kernel accumulates into and the post-pass reads, m[pair][k] = sum_n w(n) G(n) u^k,
+ * PAPER.md:238-282 (Alg. 2) -- is a static device array inside the library instead of plan-owned memory.  The call makes
+ * no cudaMalloc / cudaFree and uses no allocating library routine.
+ *   Limit: the plan's moment workspace, gpw_info.ncoef_total doubles (deriv = 2: that, rounded up to a multiple of 32,
+ *   plus the degree-(L+2) moments, about 2.4 times as much in all), must fit GPW_STATIC_MOM_DOUBLES doubles (16 MiB,
+ *   held by every GPU that loads the library until the process exits); a larger plan is rejected with GPW_EUNSUPPORTED
+ *   before anything is launched -- use gpw_eval_mat for it.
+ *   The array is one per device and shared by EVERY call and every plan; it keeps the previous call's contents, so each
+ *   call clears the part it uses on cuda_stream first.  Calls on one plan are ordered by the plan as for gpw_eval_mat;
+ *   calls on DIFFERENT plans that overlap on the GPU (different streams) race on the array -- the caller orders them.
+ */
+#define GPW_STATIC_MOM_DOUBLES (1L << 21)
+int gpw_eval_mat_static(const gpw_plan *plan, const double *const *v_dev, int deriv, double *F_dev,
+                        void *cuda_stream);
+
+/*
  * Host-buffer variants: the same two operations with every array in HOST memory (D_host [nao][nao]; rho_host /
  * v_host: HOST arrays of nlevel HOST pointers [ncomp][N1][N2][N3]; F_host [nao][nao]).  The library uploads the
  * inputs into staging buffers it owns, runs the kernels and downloads the results, on three streams of its own

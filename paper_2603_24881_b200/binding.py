@@ -58,12 +58,12 @@ _lib = None
 
 EXPORTS = ["gpw_build_pairs", "gpw_eval_rho", "gpw_eval_mat", "gpw_eval_grad", "gpw_interp_up", "gpw_restrict_down",
            "gpw_hartree", "gpw_gspace_gradient", "gpw_gspace_divergence",
-           "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait", "gpw_plan_set_partition", "gpw_plan_partition_bounds",
+           "gpw_eval_mat_static", "gpw_eval_rho_host", "gpw_eval_mat_host", "gpw_plan_wait", "gpw_plan_set_partition", "gpw_plan_partition_bounds",
            "gpw_plan_info", "gpw_plan_export_tasks", "gpw_plan_export_visits", "gpw_free_plan", "gpw_last_error", "gpw_dfma_peak", "gpw_dmma_peak",
            "gpw_plan_set_timing", "gpw_plan_get_timing"]
 
 
-__all__ = [n for n in EXPORTS if n != "gpw_last_error"] + ["GpwError", "Plan", "load_library", "model_flops", "EXPORTS"]
+__all__ = [n for n in EXPORTS if n != "gpw_last_error"] + ["GpwError", "Plan", "load_library", "model_flops", "EXPORTS", "GPW_STATIC_MOM_DOUBLES"]
 
 
 def load_library():
@@ -84,6 +84,9 @@ def load_library():
     L.gpw_eval_mat.restype = ctypes.c_int
     L.gpw_eval_mat.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
                                ctypes.c_void_p, ctypes.c_void_p]
+    L.gpw_eval_mat_static.restype = ctypes.c_int
+    L.gpw_eval_mat_static.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
+                                      ctypes.c_void_p, ctypes.c_void_p]
     L.gpw_eval_grad.restype = ctypes.c_int
     L.gpw_eval_grad.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p), ctypes.c_int,
                                 ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
@@ -243,6 +246,20 @@ def gpw_eval_mat(plan: Plan, v: Sequence, deriv: int, F, stream=None):
         _check_grid(v[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
     ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
     _check(load_library().gpw_eval_mat(plan._h, ptrs, int(deriv), ctypes.c_void_p(F.data_ptr()), _stream_ptr(stream)))
+
+
+GPW_STATIC_MOM_DOUBLES = 1 << 21
+
+
+def gpw_eval_mat_static(plan: Plan, v: Sequence, deriv: int, F, stream=None):
+    """gpw_eval_mat with the moment workspace in the library's static device array: no allocation inside the call;
+    plans whose workspace exceeds GPW_STATIC_MOM_DOUBLES are rejected (GpwError, GPW_EUNSUPPORTED)."""
+    nc = NCOMP[int(deriv)]
+    _check_grid(F, (plan.nao, plan.nao), "F")
+    for lev in range(plan.nlevel):
+        _check_grid(v[lev], (nc,) + tuple(int(x) for x in plan.mesh[lev]), f"v[{lev}]")
+    ptrs = (ctypes.c_void_p * plan.nlevel)(*[x.data_ptr() for x in v])
+    _check(load_library().gpw_eval_mat_static(plan._h, ptrs, int(deriv), ctypes.c_void_p(F.data_ptr()), _stream_ptr(stream)))
 
 
 def _check_host(t, shape, what):

@@ -555,6 +555,77 @@ int gpw_eval_grad(gpw_plan *p, const double *const *v_dev, int deriv, const doub
     return end_call(p, st, "gpw_eval_grad");
 }
 
+// ---- integration without any allocation: the moment workspace in a static device array ----
+// gpw_eval_mat's scratch is the moment vector (one block of ncoef(L + off) doubles per pair, added to atomically by
+// k_integrate, read by the post-pass).  Here it lives in the library's image: every GPU that loads the library holds
+// GPW_STATIC_MOM_DOUBLES * 8 bytes until exit.  The name below is a device symbol; host code may only use the
+// address cudaGetSymbolAddress returns for the current device.
+static __device__ __align__(256) double g_static_mom[GPW_STATIC_MOM_DOUBLES];
+
+// device address of g_static_mom on the current device, looked up once per device (with that device current)
+static int static_mom_address(double **out, const char *who) {
+    constexpr int MAXDEV = 64;
+    static double *addr[MAXDEV] = {nullptr};
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), who)) return GPW_ECUDA;
+    if (dev < 0 || dev >= MAXDEV) { set_error(std::string(who) + ": device ordinal out of range"); return GPW_EUNSUPPORTED; }
+    if (!addr[dev]) {
+        double *ptr = nullptr;
+        if (!cuda_ok(cudaGetSymbolAddress((void **)&ptr, g_static_mom), who)) return GPW_ECUDA;
+        if (!ptr) { set_error(std::string(who) + ": cudaGetSymbolAddress returned a null address"); return GPW_ECUDA; }
+        addr[dev] = ptr;
+    }
+    *out = addr[dev];
+    return GPW_OK;
+}
+
+int gpw_eval_mat_static(const gpw_plan *p, const double *const *v_dev, int deriv, double *F_dev, void *cuda_stream) {
+    const char *who = "gpw_eval_mat_static";
+    if (!p || !v_dev || !F_dev) { set_error("gpw_eval_mat_static: null argument"); return GPW_EINVAL; }
+    if (deriv < 0 || deriv > 2) { set_error("gpw_eval_mat_static: deriv must be 0, 1 or 2"); return GPW_EINVAL; }
+    if (!p->on_device) { set_error("gpw_eval_mat_static: the plan has no device copy (no CUDA device at build time); there is no CPU path"); return GPW_ECUDA; }
+    const HostPlan *hp = p->hp;
+    for (int a = 0; a < hp->nlevel; a++) {
+        if (!v_dev[a]) { set_error("gpw_eval_mat_static: null level pointer"); return GPW_EINVAL; }
+        if (!aligned16(v_dev[a])) { set_error("gpw_eval_mat_static: level pointers must be 16-byte aligned"); return GPW_EINVAL; }
+    }
+    // the moments of degree offset 0, then (deriv = 2) those of offset 2 from the next 256-byte boundary
+    const size_t n0 = (size_t)hp->ncoef_total[0];
+    const size_t off2 = (n0 + 31) / 32 * 32;
+    const size_t need = deriv == 2 ? off2 + (size_t)hp->ncoef_total[2] : n0;
+    if (need > (size_t)GPW_STATIC_MOM_DOUBLES) {
+        set_error("gpw_eval_mat_static: the plan's moment workspace (" + std::to_string(need) + " doubles) exceeds GPW_STATIC_MOM_DOUBLES (" +
+                  std::to_string((long long)GPW_STATIC_MOM_DOUBLES) + "); use gpw_eval_mat");
+        return GPW_EUNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (const int rc = begin_call(p, st, who)) return rc;
+    double *mom = nullptr;
+    if (const int rc = static_mom_address(&mom, who)) return rc;
+    if (!cuda_ok(cudaMemsetAsync(F_dev, 0, sizeof(double) * (size_t)hp->nao * hp->nao, st), "gpw_eval_mat_static: memset")) return GPW_ECUDA;
+    const int ntask = (int)hp->ntask, nitem = (int)hp->nitem;
+    if (ntask == 0 || nitem == 0) return end_call(p, st, who);
+    // the array keeps the previous call's moments: clear the part this call accumulates into
+    if (!cuda_ok(cudaMemsetAsync(mom, 0, sizeof(double) * need, st), "gpw_eval_mat_static: memset")) return GPW_ECUDA;
+    GridParams P;
+    fill_params(p, P, const_cast<double *const *>(v_dev));
+    if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, mom, deriv ? 1 : 0, 0,
+                                  hp->max_L, hp->ortho, st), "gpw_eval_mat_static: integration launch")) return GPW_ECUDA;
+    if (deriv == 2) {
+        fill_params(p, P, const_cast<double *const *>(v_dev), 2, 4);
+        if (!cuda_ok(launch_integrate(P, p->d_taskK, p->lists.bentry, p->lists.bitem, (int)hp->nbitem, p->d_eg, mom + off2, 0, 2,
+                                      hp->max_L, hp->ortho, st), "gpw_eval_mat_static: kinetic-energy integration launch")) return GPW_ECUDA;
+    }
+    pp::PassArgs A;
+    fill_pass(p, A, pp::POST_MAT | (deriv == 2 ? pp::POST_TAU : 0));
+    A.mom[0] = mom;
+    A.mom[2] = deriv == 2 ? mom + off2 : nullptr;
+    A.F = F_dev;
+    if (!cuda_ok(launch_pair_pass(A, hp->max_l, hp->max_L, st), "gpw_eval_mat_static: post-pass launch")) return GPW_ECUDA;
+    if (!cuda_ok(cudaGetLastError(), "gpw_eval_mat_static: kernel launch")) return GPW_ECUDA;
+    return end_call(p, st, who);
+}
+
 // ---- host-buffer variants ----
 static int ensure_hostio(gpw_plan *p, int ncomp, const char *who) {
     const HostPlan *hp = p->hp;
