@@ -253,13 +253,12 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         }
     };
     if constexpr (LMAX <= 4 || DERIV == 0) {
-        static_assert(LLO == 0, "the straight-line form starts at L = 0");
-        run_segment(std::integral_constant<int, 0>{}, kend[0]);
-        run_segment(std::integral_constant<int, 1>{}, kend[1]);
-        run_segment(std::integral_constant<int, 2>{}, kend[2]);
-        if constexpr (LMAX >= 3) run_segment(std::integral_constant<int, 3>{}, kend[3]);
-        if constexpr (LMAX >= 4) run_segment(std::integral_constant<int, 4>{}, kend[4]);
-        if constexpr (LMAX >= 5) run_segment(std::integral_constant<int, 5>{}, kend[5]);
+        if constexpr (LLO <= 0) run_segment(std::integral_constant<int, 0>{}, kend[0]);
+        if constexpr (LLO <= 1) run_segment(std::integral_constant<int, 1>{}, kend[1]);
+        if constexpr (LLO <= 2) run_segment(std::integral_constant<int, 2>{}, kend[2]);
+        if constexpr (LMAX >= 3 && LLO <= 3) run_segment(std::integral_constant<int, 3>{}, kend[3]);
+        if constexpr (LMAX >= 4 && LLO <= 4) run_segment(std::integral_constant<int, 4>{}, kend[4]);
+        if constexpr (LMAX >= 5 && LLO <= 5) run_segment(std::integral_constant<int, 5>{}, kend[5]);
         if constexpr (LMAX >= 6) run_segment(std::integral_constant<int, 6>{}, kend[6]);
     } else {
         // deriv = 1 with f shells (L up to 6): the straight-line form costs registers the L = 5, 6 bodies do not
@@ -342,15 +341,19 @@ cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, 
 }
 
 template <int DERIV, bool ORTHO>
-cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+cudaError_t launch_l(const GridParams &P, const Visit *visits, const Item *items, int nitem, const Item *items_hi, int nitem_hi,
                      const double *rec, const double *vg, int max_L, cudaStream_t st) {
     if (max_L <= 2) return launch<DERIV, 2, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
     if (max_L <= 4) return launch<DERIV, 4, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
     if constexpr (DERIV != 0) {   // two launches: classes L <= 4, then L = 5, 6 on top (see k_collocate): cfg4 28.9 -> 24.6 ms
         const cudaError_t e = launch<DERIV, 4, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
         if (e != cudaSuccess) return e;
-        return launch<DERIV, 6, ORTHO, 0, 5, true>(P, visits, items, nitem, rec, vg, st);
+        // ... over its own items (the tails L >= 5 of the blocks' lists): on cfg 4 nine items in ten of the full list hold
+        // no such visit, and 700 000 warps that only find that out cost more than the work of the others
+        if (nitem_hi <= 0) return cudaSuccess;
+        return launch<DERIV, 6, ORTHO, 0, 5, true>(P, visits, items_hi, nitem_hi, rec, vg, st);
     } else {
+        // (two launches like the above, with the second over its own items, were measured for deriv = 0 too: cfg 3 1.45 -> 1.46 ms)
         return launch<DERIV, 6, ORTHO, 0>(P, visits, items, nitem, rec, vg, st);
     }
 }
@@ -365,15 +368,16 @@ cudaError_t launch_tau(const GridParams &P, const Visit *visits, const Item *ite
 }  // namespace
 
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                             const Item *items_hi, int nitem_hi,
                              const double *rec, const double *vg, int deriv, int off, int max_L, bool ortho, cudaStream_t st) {
     if (off == 2 && deriv == 0)
         return ortho ? launch_tau<true>(P, visits, items, nitem, rec, vg, max_L, st)
                      : launch_tau<false>(P, visits, items, nitem, rec, vg, max_L, st);
     if (off != 0) return cudaErrorInvalidValue;
-    if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, rec, vg, max_L, st)
-                            : launch_l<1, false>(P, visits, items, nitem, rec, vg, max_L, st);
-    return ortho ? launch_l<0, true>(P, visits, items, nitem, rec, vg, max_L, st)
-                 : launch_l<0, false>(P, visits, items, nitem, rec, vg, max_L, st);
+    if (deriv) return ortho ? launch_l<1, true>(P, visits, items, nitem, items_hi, nitem_hi, rec, vg, max_L, st)
+                            : launch_l<1, false>(P, visits, items, nitem, items_hi, nitem_hi, rec, vg, max_L, st);
+    return ortho ? launch_l<0, true>(P, visits, items, nitem, items_hi, nitem_hi, rec, vg, max_L, st)
+                 : launch_l<0, false>(P, visits, items, nitem, items_hi, nitem_hi, rec, vg, max_L, st);
 }
 
 // ---------------------------------------------------------------------------------------- plan-time kernel

@@ -477,11 +477,12 @@ int gpw_eval_rho(const gpw_plan *p, const double *D_dev, int deriv, double *cons
     if (p->timing) cudaEventRecord(p->ev[0][1], st);
     GridParams P;
     fill_params(p, P, rho_dev);
-    if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef[0], p->d_vg, deriv ? 1 : 0, 0, hp->max_L, hp->ortho, st),
+    if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->lists.item_hi, (int)p->lists.nitem_hi, p->d_coef[0], p->d_vg,
+                                  deriv ? 1 : 0, 0, hp->max_L, hp->ortho, st),
                  "gpw_eval_rho: collocation launch")) return GPW_ECUDA;
     if (deriv == 2) {   // fifth component: tau, polynomials of degree L + 2, value only (Eq. 15)
         fill_params(p, P, rho_dev, 2, 4);
-        if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, p->d_coef[2], p->d_vg, 0, 2, hp->max_L, hp->ortho, st),
+        if (!cuda_ok(launch_collocate(P, p->lists.visit, p->lists.item, nitem, nullptr, 0, p->d_coef[2], p->d_vg, 0, 2, hp->max_L, hp->ortho, st),
                      "gpw_eval_rho: kinetic-energy collocation launch")) return GPW_ECUDA;
     }
     if (p->timing) cudaEventRecord(p->ev[0][2], st);

@@ -41,7 +41,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // vg: Gaussian values of every visit (visit_gauss_doubles(ortho) per visit, order of `visits`), written once per
 // plan by launch_visit_gauss
 // off: degree offset of the launch (0, or 2 with deriv = 0: kinetic-energy density); rec and P.coef_base are those of `off`
+// items_hi: the items over the visits of the classes L >= 5 alone (plans with f shells; the second launch of deriv = 1)
 cudaError_t launch_collocate(const GridParams &P, const Visit *visits, const Item *items, int nitem,
+                             const Item *items_hi, int nitem_hi,
                              const double *rec, const double *vg, int deriv, int off, int max_L, bool ortho, cudaStream_t st);
 size_t visit_gauss_doubles(bool ortho);
 cudaError_t launch_visit_gauss(const GridParams &P, int ntile_all, const TaskK *tasks, const Visit *visits, double *vg,

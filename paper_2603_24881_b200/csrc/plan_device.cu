@@ -185,28 +185,33 @@ __device__ __forceinline__ int level_of(const ListGeom &G, long long id, bool br
 }
 
 // ---------------------------------------------------------------------------------------- work items
-__global__ void k_items_count(const long long *__restrict__ base, long long nblock, unsigned *__restrict__ nparts, unsigned maxlen) {
+// seg != nullptr: only the tail of every block's list that starts at its segment llo (classes L >= llo)
+__global__ void k_items_count(const long long *__restrict__ base, long long nblock, unsigned *__restrict__ nparts, unsigned maxlen,
+                              const unsigned *__restrict__ seg = nullptr, int llo = 0) {
     const long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (b >= nblock) return;
-    const unsigned n = (unsigned)(base[b + 1] - base[b]);
+    unsigned n = (unsigned)(base[b + 1] - base[b]);
+    if (seg) n -= seg[b * 8 + llo];
     nparts[b] = (n + maxlen - 1) / maxlen;
 }
 
 __global__ void k_items_fill(const __grid_constant__ ListGeom G, const long long *__restrict__ base, long long nblock,
                              const unsigned *__restrict__ nparts, const long long *__restrict__ off,
-                             unsigned *__restrict__ key, Item *__restrict__ items) {
+                             unsigned *__restrict__ key, Item *__restrict__ items,
+                             const unsigned *__restrict__ seg = nullptr, int llo = 0) {
     const long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (b >= nblock) return;
     const unsigned np = nparts[b];
     if (!np) return;
-    const unsigned n = (unsigned)(base[b + 1] - base[b]);
+    const unsigned first = seg ? seg[b * 8 + llo] : 0u;   // the items cover [first, end of the block's list)
+    const unsigned n = (unsigned)(base[b + 1] - base[b]) - first;
     long long local;
     const int level = level_of(G, b, false, &local);
     for (unsigned p = 0; p < np; p++) {
         Item it;
         it.level = level; it.tile = (int)local;
-        it.lo = (unsigned)((unsigned long long)n * p / np);
-        it.hi = (unsigned)((unsigned long long)n * (p + 1) / np);
+        it.lo = first + (unsigned)((unsigned long long)n * p / np);
+        it.hi = first + (unsigned)((unsigned long long)n * (p + 1) / np);
         it.single = np == 1; it.pad = 0;
         it.vstart = base[b] + it.lo;
         items[off[b] + p] = it;
@@ -325,7 +330,8 @@ int bits_for(unsigned long long maxval) {
 
 void free_device_lists(DeviceLists *l) {
     if (!l) return;
-    cudaFree(l->visit); cudaFree(l->tile_base); cudaFree(l->seg); cudaFree(l->item);
+    cudaFree(l->visit); cudaFree(l->tile_base); cudaFree(l->seg); cudaFree(l->item); cudaFree(l->item_hi);
+    l->item_hi = nullptr; l->nitem_hi = 0;
     cudaFree(l->bentry); cudaFree(l->brick_base); cudaFree(l->bitem);
     l->visit = nullptr; l->tile_base = nullptr; l->seg = nullptr; l->item = nullptr;
     l->bentry = nullptr; l->brick_base = nullptr; l->bitem = nullptr;
@@ -366,7 +372,8 @@ int build_device_lists(const HostPlan *hp, const DevTask *d_task, int ntask, Dev
         out->tile_base = tb; out->seg = sg; out->brick_base = bb;
     }
     auto give_up = [&](int rc) { out->tile_base = nullptr; out->seg = nullptr; out->brick_base = nullptr; out->visit = nullptr;
-                                 out->item = nullptr; out->bentry = nullptr; out->bitem = nullptr; return rc; };
+                                 out->item = nullptr; out->item_hi = nullptr; out->nitem_hi = 0;
+                                 out->bentry = nullptr; out->bitem = nullptr; return rc; };
     if (ntask == 0) {
         cudaMemsetAsync(out->tile_base, 0, sizeof(long long) * ((size_t)ntile_all + 1), st);
         cudaMemsetAsync(out->seg, 0, sizeof(unsigned) * (size_t)ntile_all * 8, st);
@@ -438,6 +445,29 @@ int build_device_lists(const HostPlan *hp, const DevTask *d_task, int ntask, Dev
             S.free_now(np); S.free_now(ioff); S.free_now(ikey); S.free_now(ikey2); S.free_now(it);
             out->item = it2; out->nitem = (long)nitem;
         }
+        // ---- ... and, on plans with f shells, the items of the second collocation launch: the visits of the classes
+        //      L >= 5 (the tail of every block's list), so that the launch holds no item without work ----
+        if (hp->max_L >= 5) {
+            unsigned *np = nullptr, *ikey = nullptr, *ikey2 = nullptr;
+            long long *ioff = nullptr;
+            Item *it = nullptr, *it2 = nullptr;
+            GPW_ALLOC(&np, (size_t)ntile_all, "items"); GPW_ALLOC(&ioff, (size_t)ntile_all, "items");
+            k_items_count<<<(unsigned)((ntile_all + 255) / 256), 256, 0, st>>>(out->tile_base, ntile_all, np, ITEM_MAX, out->seg, 5);
+            GPW_TRY(cudaGetLastError(), "items");
+            long long nitem = 0;
+            if ((rc = scan_counts(S, np, ntile_all, ioff, &nitem, st)) != GPW_OK) return rc;
+            if (nitem > 0) {
+                GPW_ALLOC(&ikey, (size_t)nitem, "items"); GPW_ALLOC(&ikey2, (size_t)nitem, "items");
+                GPW_ALLOC(&it, (size_t)nitem, "items");
+                if (!S.alloc(&it2, (size_t)nitem, &nb)) return fail("items", cudaErrorMemoryAllocation);
+                k_items_fill<<<(unsigned)((ntile_all + 255) / 256), 256, 0, st>>>(G, out->tile_base, ntile_all, np, ioff, ikey, it, out->seg, 5);
+                GPW_TRY(cudaGetLastError(), "items");
+                if ((rc = sort_pairs(S, ikey, ikey2, it, it2, nitem, bits_for(ITEM_MAX), st)) != GPW_OK) return rc;
+                S.free_now(ikey); S.free_now(ikey2); S.free_now(it);
+                out->item_hi = it2; out->nitem_hi = (long)nitem;
+            }
+            S.free_now(np); S.free_now(ioff);
+        }
         S.free_now(vkey2);
         out->visit = reinterpret_cast<Visit *>(vval2);
         // ---- brick entries: stable sort by (brick, L, blocks visited descending) ----
@@ -480,6 +510,7 @@ int build_device_lists(const HostPlan *hp, const DevTask *d_task, int ntask, Dev
     if (rc != GPW_OK) return give_up(rc);   // Scratch frees everything, including what `out` pointed at
     S.release(out->tile_base); S.release(out->seg); S.release(out->brick_base);
     S.release(out->visit); S.release(out->item); S.release(out->bentry); S.release(out->bitem);
+    if (out->item_hi) S.release(out->item_hi);
     out->seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
     return GPW_OK;
 }

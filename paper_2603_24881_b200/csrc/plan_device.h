@@ -32,6 +32,8 @@ struct DeviceLists {
     unsigned *seg = nullptr;             // [ntile_all * 8] start of each L segment relative to the block's list
     Item *item = nullptr;
     long nitem = 0;
+    Item *item_hi = nullptr;             // items over the visits of the classes L >= 5 only (second collocation launch of
+    long nitem_hi = 0;                   // plans with f shells): the blocks that have such visits, nothing else
     BEntry *bentry = nullptr;            // [nentry] brick-major, inside a brick by L then by decreasing blocks
     long long nentry = 0;
     long long *brick_base = nullptr;     // [nbrick_all + 1]
