@@ -27,7 +27,14 @@ constexpr int NGRP = 8;     // groups of 4 lanes per warp
 // finishes, instead of waiting for the slowest of four items (measured: cfg2 k_collocate 3.58 -> 3.47 ms,
 // cfg4 30.8 -> 29.6 ms; two warps per CTA: no gain)
 constexpr int NWARP = 1;
-constexpr int NSLOT = 3;    // shared-memory slots per group (copy issued two chunks ahead)
+// Shared-memory slots per group: three (copy issued two chunks ahead), except where the slots are what limits the
+// resident warps -- value-only launches with polynomials of degree >= 5 (168 registers or fewer allow twelve warps per
+// SM, three slots of 100-186 doubles per group only nine, or five for the degree-8 polynomials of tau): two there, the
+// copy one chunk ahead.
+#ifndef GPW_NSLOT_SMALL
+#define GPW_NSLOT_SMALL 2
+#endif
+GPW_CX int nslot(int deriv, int dmax) { return (deriv == 0 && dmax >= 5) ? GPW_NSLOT_SMALL : 3; }
 constexpr int MAXCH = 64;   // chunks per item: ITEM_MAX / NGRP full ones + one ragged chunk per L segment
 constexpr int MAXVIS = 384; // visits per item (ITEM_MAX of plan.cpp)
 
@@ -40,13 +47,13 @@ GPW_CX int slot_vg(int lmax) { return 8 + ncoef_pad(lmax); }
 GPW_CX int slot_doubles(int lmax, bool ortho) { return slot_vg(lmax) + vg_doubles(ortho); }
 // A group's slots, padded to an odd number of 16-byte units: the eight groups' broadcast reads of the same
 // coefficient then hit eight different bank pairs.
-GPW_CX int group_stride(int lmax, bool ortho) {
-    int n = NSLOT * slot_doubles(lmax, ortho);
+GPW_CX int group_stride(int lmax, bool ortho, int ns) {
+    int n = ns * slot_doubles(lmax, ortho);
     while (n % 4 != 2) n += 2;
     return n;
 }
 // per warp: the groups' slots, the chunk table, the item's visit records
-GPW_CX int warp_doubles(int lmax, bool ortho) { return NGRP * group_stride(lmax, ortho) + MAXCH + MAXVIS; }
+GPW_CX int warp_doubles(int lmax, bool ortho, int ns) { return NGRP * group_stride(lmax, ortho, ns) + MAXCH + MAXVIS; }
 
 struct ColCtx {
     const double *rec;     // per-pair records: header (8 doubles) + polynomial
@@ -142,7 +149,8 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
     constexpr int NCOMP = DERIV ? 4 : 1;
     constexpr int DMAX = LMAX + LOFF;
     constexpr int SLOT = slot_doubles(DMAX, ORTHO);
-    constexpr int GSTRIDE = group_stride(DMAX, ORTHO);
+    constexpr int NSLOT = nslot(DERIV, DMAX);
+    constexpr int GSTRIDE = group_stride(DMAX, ORTHO, NSLOT);
     extern __shared__ __align__(16) double sm[];
     const int warp = threadIdx.x >> 5;
     const int w = blockIdx.x * NWARP + warp;
@@ -154,7 +162,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         if (b1 < P.part_lo[it.level] || b1 >= P.part_hi[it.level]) return;
     }
     const int lane = threadIdx.x & 31, grp = lane >> 2, x = lane & 3;
-    double *wsm = sm + (size_t)warp * warp_doubles(DMAX, ORTHO);
+    double *wsm = sm + (size_t)warp * warp_doubles(DMAX, ORTHO, NSLOT);
     uint2 *tab = reinterpret_cast<uint2 *>(wsm + NGRP * GSTRIDE);
     unsigned long long *vis = reinterpret_cast<unsigned long long *>(wsm + NGRP * GSTRIDE + MAXCH);
 
@@ -225,7 +233,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         cp_async_commit();
     };
     stage_chunk(0, 0);
-    stage_chunk(1, 1);
+    if constexpr (NSLOT > 2) stage_chunk(1, 1);
     // One loop per L segment, its body straight-line code: a group without a visit of its own in a ragged chunk
     // evaluates group 0's visit with a zero Gaussian instead of branching around the evaluation, so that the
     // control work of the next chunks (table and visit records, cp.async addresses) can be scheduled into the
@@ -240,9 +248,9 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         constexpr int L = decltype(Lc)::value;
 #pragma unroll 1
         for (; k < k_end; k++) {
-            cp_async_wait<1>();   // chunk k has landed (chunk k+1 may still be in flight)
+            cp_async_wait<NSLOT - 2>();   // chunk k has landed (with three slots chunk k+1 may still be in flight)
             __syncwarp();         // ... for all four lanes of the group; and every lane has left the slot refilled next
-            stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
+            stage_chunk(k + NSLOT - 1, slot >= 1 ? slot - 1 : slot + NSLOT - 1);
             const uint2 en = tab[min(k + 1, nch - 1)];
             const bool valid_n = (unsigned)grp < (en.y >> 8);
             const int gi_n = valid_n ? grp : 0;
@@ -265,9 +273,9 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
         // have (measured on cfg 4: 7 % slower); one loop, the evaluation behind a branch
 #pragma unroll 1
         for (; k < nch; k++) {
-            cp_async_wait<1>();
+            cp_async_wait<NSLOT - 2>();
             __syncwarp();
-            stage_chunk(k + 2, slot >= 1 ? slot - 1 : slot + 2);
+            stage_chunk(k + NSLOT - 1, slot >= 1 ? slot - 1 : slot + NSLOT - 1);
             const uint2 e = tab[k];
             if ((unsigned)grp < (e.y >> 8)) {
                 const unsigned long long v0 = vis[e.x + grp];
@@ -325,7 +333,7 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV ? 8 : 12) / NWARP) k_colloc
 template <int DERIV, int LMAX, bool ORTHO, int LOFF, int LLO = 0, bool ACC = false>
 cudaError_t launch(const GridParams &P, const Visit *visits, const Item *items, int nitem,
                    const double *rec, const double *vg, cudaStream_t st) {
-    constexpr int smem = NWARP * warp_doubles(LMAX + LOFF, ORTHO) * (int)sizeof(double);
+    constexpr int smem = NWARP * warp_doubles(LMAX + LOFF, ORTHO, nslot(DERIV, LMAX + LOFF)) * (int)sizeof(double);
     // the attribute is per device (and per instantiation)
     static bool configured_dev[64] = {false};
     int dev = -1;
