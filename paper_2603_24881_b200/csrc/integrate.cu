@@ -116,23 +116,58 @@ __device__ __forceinline__ void integ_entry(const BrickCtx &c, const BEntry en, 
         }
     }
     __syncwarp();
-    // expansion in u1, sum over the group's four lanes (n1 planes), one atomic per moment
+    // expansion in u1, sum over the group's four lanes (n1 planes), one atomic per moment.  The sum is a reduce-scatter:
+    // after the exchange with lane x ^ 1 a lane holds the pair sums of one half of the moments, after the one with lane
+    // x ^ 2 the full sums of one quarter, which it adds to the workspace -- 3/4 N shuffles of doubles instead of the 2 N
+    // of a butterfly per moment (the shuffles share the shared-memory pipe the block loops are bound by; the entry tails
+    // were 12 % of the warp samples of cfg 2).  Same summation tree: (x0 + x1) + (x2 + x3).
+    constexpr int N = ncoef(L), N4 = (N + 3) & ~3, HALF = N4 / 2, QUART = N4 / 4;
     double pw1[L + 1];
     pw1[0] = 1.0;
 #pragma unroll
     for (int k = 1; k <= L; k++) pw1[k] = pw1[k - 1] * u1;
+    if constexpr (N > 84) {
+        // degree 7, 8 (the derivative variants of f shells): 120 / 165 moments do not fit a register array; a butterfly per moment
+#pragma unroll
+        for (int kz = 0; kz <= L; kz++)
+#pragma unroll
+            for (int ky = 0; ky <= L - kz; ky++)
+#pragma unroll
+                for (int kx = 0; kx <= L - kz - ky; kx++) {
+                    double s = integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
+                    s += __shfl_xor_sync(0xffffffffu, s, 1);
+                    s += __shfl_xor_sync(0xffffffffu, s, 2);
+                    const int k = cidx(L, kx, ky, kz);
+                    if (valid && (k & 3) == c.x) atomicAdd(dst + k, s);
+                }
+        return;
+    }
+    double sv[N4];
+#pragma unroll
+    for (int k = N; k < N4; k++) sv[k] = 0.0;
 #pragma unroll
     for (int kz = 0; kz <= L; kz++)
 #pragma unroll
         for (int ky = 0; ky <= L - kz; ky++)
 #pragma unroll
-            for (int kx = 0; kx <= L - kz - ky; kx++) {
-                double s = integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
-                s += __shfl_xor_sync(0xffffffffu, s, 1);
-                s += __shfl_xor_sync(0xffffffffu, s, 2);
-                const int k = cidx(L, kx, ky, kz);
-                if (valid && (k & 3) == c.x) atomicAdd(dst + k, s);
-            }
+            for (int kx = 0; kx <= L - kz - ky; kx++) sv[cidx(L, kx, ky, kz)] = integ_expand_term<L, DERIV>(B0, B1, pw1, kx, ky, kz);
+    const bool up1 = c.x & 1, up2 = c.x & 2;
+#pragma unroll
+    for (int i = 0; i < HALF; i++) {
+        const double send = up1 ? sv[i] : sv[i + HALF];
+        const double keep = up1 ? sv[i + HALF] : sv[i];
+        sv[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+    }
+#pragma unroll
+    for (int i = 0; i < QUART; i++) {
+        const double send = up2 ? sv[i] : sv[i + QUART];
+        const double keep = up2 ? sv[i + QUART] : sv[i];
+        sv[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+    }
+    const int off = (up1 ? HALF : 0) + (up2 ? QUART : 0);
+#pragma unroll
+    for (int i = 0; i < QUART; i++)
+        if (valid && off + i < N) atomicAdd(dst + off + i, sv[i]);
 }
 
 // LMAX: largest la + lb held by the instantiation.  LOFF: degree offset -- the moments of a pair of class L are
