@@ -208,22 +208,26 @@ __global__ void __launch_bounds__(NWARP * 32, (DERIV || LMAX + LOFF > 4) ? 2 : 3
     }
 
     // The item's entries in chunks of NGRP that never straddle an L segment (so the code path is
-    // warp-uniform); the chunks are dealt to the CTA's warps round robin.
-    int L = LLO - 1, cc = 0;
-    unsigned base = 0, hi = 0;
+    // warp-uniform); the chunks are dealt to the CTA's warps round robin: warp w takes the chunks w, w + NWARP, ... of
+    // the item's chunk sequence and finds each by walking the segments forward (chunk c lies in the segment whose
+    // first chunk c0 and chunk count n have c0 <= c < c0 + n).
+    int L = LLO - 1, cnext = warp, kc0 = 0, nseg = 0;
+    unsigned base = 0, lo = 0, hi = 0;
     auto next_chunk = [&]() -> bool {
-        for (;;) {
-            base += NGRP;
-            if (L < LLO || base >= hi) {
-                do {
-                    L++;
-                    if (L > LMAX) return false;
-                    base = max(it_lo, s_seg[L]);
-                    hi = min(it_hi, s_seg[L + 1]);
-                } while (base >= hi);
-            }
-            if ((cc++ % NWARP) == warp) return true;
+        if (L > LMAX) return false;   // past the last segment (the sequence has ended for this warp)
+        const int cidx_ = cnext;
+        cnext += NWARP;
+        while (cidx_ >= kc0 + nseg) {
+            kc0 += nseg;
+            nseg = 0;
+            L++;
+            if (L > LMAX) return false;
+            lo = max(it_lo, s_seg[L]);
+            hi = min(it_hi, s_seg[L + 1]);
+            nseg = lo < hi ? (int)((hi - lo + NGRP - 1) / NGRP) : 0;
         }
+        base = lo + (unsigned)(NGRP * (cidx_ - kc0));
+        return true;
     };
     // Software pipeline over the warp's chunks: the entry records are loaded two chunks ahead (one 16-byte load
     // per group), the pair records, whose address depends on the entry, one chunk ahead.
