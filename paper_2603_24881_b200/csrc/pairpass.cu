@@ -16,14 +16,16 @@ using namespace pp;
 constexpr int PP_THREADS = 128;
 constexpr int PP_GROUPS = PP_THREADS / PP_G;
 
-// LS: the largest shell angular momentum the instantiation holds: q [ncart(LS)][ncoef(LS)], R of degree 2 LS + 2
+// LS: the largest shell angular momentum the instantiation holds: q [ncart(LS)][ncoef(LS)], R of degree 2 LS + off, off the
+// largest degree offset of the launch's modes (0: density / Fock matrix, 1: nuclear gradient, 2: tau) -- sized per launch,
+// because the shared memory is what limits the resident groups (LS = 3: 285 doubles per group on the hot path, 366 for tau)
 template <int LS>
-GPW_CX int group_doubles() { return ncart(LS) * ncoef(LS) + ncoef(2 * LS + NOFF - 1) + 1; }   // odd: groups start in different banks
+GPW_CX int group_doubles(int off) { return ncart(LS) * ncoef(LS) + ncoef(2 * LS + off) + 1; }
 
 __device__ Tables d_tables;   // index tables (pairpass.cuh), written once per process and device by upload_tables
 
 template <int LS>
-__global__ void __launch_bounds__(PP_THREADS) k_pair_pass(const __grid_constant__ PassArgs A) {
+__global__ void __launch_bounds__(PP_THREADS) k_pair_pass(const __grid_constant__ PassArgs A, int gdoubles) {
     extern __shared__ double sm[];
     __shared__ Tables s_tab;
     {
@@ -44,7 +46,7 @@ __global__ void __launch_bounds__(PP_THREADS) k_pair_pass(const __grid_constant_
     g.G = PP_G;
     g.mask = 0xffu << (8 * ((threadIdx.x & 31) / PP_G));
     g.tab = &s_tab;
-    double *q = sm + (size_t)grp * group_doubles<LS>();
+    double *q = sm + (size_t)grp * gdoubles;
     pair_pass<ncoef(LS)>(A, t, q, q + ncart(LS) * ncoef(LS), g);
 }
 
@@ -98,8 +100,15 @@ cudaError_t launch_pair_pass(const pp::PassArgs &A0, int max_l, int max_L, cudaS
     }
     if (A.nsel == 0) return cudaSuccess;
     const int nblk = (A.nsel + PP_GROUPS - 1) / PP_GROUPS;
-    if (max_l <= 2) k_pair_pass<2><<<nblk, PP_THREADS, PP_GROUPS * group_doubles<2>() * sizeof(double), st>>>(A);
-    else k_pair_pass<3><<<nblk, PP_THREADS, PP_GROUPS * group_doubles<3>() * sizeof(double), st>>>(A);
+    const int off = (A.mode & (PRE_TAU | POST_TAU)) ? 2 : ((A.mode & POST_GRAD) ? 1 : 0);
+    static_assert(NOFF == 3, "degree offsets 0, 1, 2");
+    if (max_l <= 2) {
+        const int gd = group_doubles<2>(off);
+        k_pair_pass<2><<<nblk, PP_THREADS, PP_GROUPS * gd * sizeof(double), st>>>(A, gd);
+    } else {
+        const int gd = group_doubles<3>(off);
+        k_pair_pass<3><<<nblk, PP_THREADS, PP_GROUPS * gd * sizeof(double), st>>>(A, gd);
+    }
     return cudaGetLastError();
 }
 
